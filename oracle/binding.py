@@ -1,0 +1,145 @@
+"""Builds (gcc) and loads liboracle.so; argument marshalling only.  TEST INFRASTRUCTURE."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nbsdf_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+# wire format of the inputs (query = position, size, wi, wo + material latent id)
+QUERY_DTYPE = np.dtype([("u", "<f4"), ("v", "<f4"), ("footprint", "<f4"), ("material", "<i4"),
+                        ("wi", "<f4", (3,)), ("wo", "<f4", (3,))], align=False)
+LIGHT_DTYPE = np.dtype([("type", "<i4"), ("vec", "<f4", (3,)), ("rgb", "<f4", (3,)),
+                        ("emit_n", "<f4", (3,))], align=False)
+assert QUERY_DTYPE.itemsize == 40 and LIGHT_DTYPE.itemsize == 40
+
+
+class _Dims(C.Structure):
+    _fields_ = [("latent_dim", C.c_int32), ("hidden", C.c_int32), ("feat_dim", C.c_int32),
+                ("n_materials", C.c_int32)]
+
+
+def build(force=False):
+    """Compile the oracle with gcc (no fast-math, no contraction).  Building is not using."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        lib.oracle_softplus.restype = C.c_double
+        lib.oracle_softplus.argtypes = [C.c_double]
+        lib.oracle_wrap.restype = C.c_double
+        lib.oracle_wrap.argtypes = [C.c_double]
+        lib.oracle_log_footprint.restype = C.c_double
+        lib.oracle_log_footprint.argtypes = [C.c_double]
+        lib.oracle_to_local.restype = None
+        lib.oracle_to_local.argtypes = [C.c_void_p] * 4
+        lib.oracle_eval.restype = C.c_int
+        lib.oracle_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                    C.c_int64, C.c_void_p, C.c_int]
+        lib.oracle_shade_frame.restype = C.c_int
+        lib.oracle_shade_frame.argtypes = [C.c_void_p] * 8 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                                              C.c_int, C.c_void_p, C.c_int]
+        lib.oracle_max_threads.restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _pack_net(weights, biases, latents):
+    """weights/biases: 6 arrays, W_k row-major [out][in]; latents [M][L].  Shapes define the dims."""
+    Ws = [_f32(w) for w in weights]
+    bs = [_f32(b).reshape(-1) for b in biases]
+    Z = _f32(latents)
+    assert len(Ws) == 6 and len(bs) == 6 and Z.ndim == 2
+    M, L = Z.shape
+    H, F = Ws[0].shape[0], Ws[2].shape[0]
+    shapes = [(H, L + 3), (H, H), (F, H), (H, F + 6), (H, H), (3, H)]
+    for w, b, s in zip(Ws, bs, shapes):
+        assert w.shape == s and b.shape == (s[0],), (w.shape, b.shape, s)
+    dims = _Dims(L, H, F, M)
+    Wp = (C.c_void_p * 6)(*[w.ctypes.data for w in Ws])
+    bp = (C.c_void_p * 6)(*[b.ctypes.data for b in bs])
+    return dims, Wp, bp, Z, (Ws, bs)
+
+
+def eval_queries(weights, biases, latents, queries, frames=None, n_threads=0):
+    """fp64 decoder over a batch of QUERY_DTYPE records -> float64 [n][3]."""
+    dims, Wp, bp, Z, _keep = _pack_net(weights, biases, latents)
+    q = np.ascontiguousarray(queries, dtype=QUERY_DTYPE)
+    n = q.shape[0]
+    fr = None
+    if frames is not None:
+        fr = _f32(frames)
+        assert fr.shape == (n, 6)
+    mats = q["material"]
+    assert n == 0 or int(mats.max()) < Z.shape[0], "material id out of range"
+    out = np.empty((n, 3), dtype=np.float64)
+    rc = _load().oracle_eval(C.byref(dims), Wp, bp, Z.ctypes.data, q.ctypes.data,
+                             fr.ctypes.data if fr is not None else None, n, out.ctypes.data, int(n_threads))
+    assert rc == 0
+    return out
+
+
+def shade_frame(weights, biases, latents, gbuffer, lights, first=0, count=None, n_threads=0):
+    """fp64 frame shading.  gbuffer: dict(pos_fp, nrm_u, tan_v [h*w][4] f32, material [h*w] i32, cam_pos[3]).
+    Returns float64 [count][3] for pixels [first, first+count)."""
+    dims, Wp, bp, Z, _keep = _pack_net(weights, biases, latents)
+    pos = _f32(gbuffer["pos_fp"]).reshape(-1, 4)
+    nrm = _f32(gbuffer["nrm_u"]).reshape(-1, 4)
+    tan = _f32(gbuffer["tan_v"]).reshape(-1, 4)
+    mat = np.ascontiguousarray(gbuffer["material"], dtype=np.int32).reshape(-1)
+    npx = mat.shape[0]
+    assert pos.shape[0] == npx and nrm.shape[0] == npx and tan.shape[0] == npx
+    cam = _f32(gbuffer["cam_pos"]).reshape(3)
+    lt = np.ascontiguousarray(lights, dtype=LIGHT_DTYPE).reshape(-1)
+    if count is None:
+        count = npx - first
+    assert 0 <= first and first + count <= npx
+    assert npx == 0 or int(mat.max()) < Z.shape[0], "material id out of range"
+    out = np.empty((count, 3), dtype=np.float64)
+    rc = _load().oracle_shade_frame(C.byref(dims), Wp, bp, Z.ctypes.data, pos.ctypes.data, nrm.ctypes.data,
+                                    tan.ctypes.data, mat.ctypes.data, first, count, cam.ctypes.data,
+                                    lt.ctypes.data if lt.shape[0] else None, lt.shape[0], out.ctypes.data,
+                                    int(n_threads))
+    assert rc == 0
+    return out
+
+
+def softplus(x):
+    return _load().oracle_softplus(float(x))
+
+
+def wrap(x):
+    return _load().oracle_wrap(float(x))
+
+
+def log_footprint(x):
+    return _load().oracle_log_footprint(float(x))
+
+
+def to_local(n, t, w):
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    out = np.empty(3, dtype=np.float64)
+    _load().oracle_to_local(n.ctypes.data, t.ctypes.data, w.ctypes.data, out.ctypes.data)
+    return out
+
+
+def max_threads():
+    return int(_load().oracle_max_threads())

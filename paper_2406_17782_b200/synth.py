@@ -1,0 +1,186 @@
+"""Seeded synthetic inputs for the decoder hot path -- data only, none of the method's arithmetic.
+
+These inputs stand in for the paper's four Falcor scenes, its trained 64-d latents and its
+1920x1080 single-light workload, none of which are available.
+Shapes and ranges follow BASELINE.json ``configs`` (which echo Table 2, PAPER.md:210-220:
+position in (0,1)^2 of the pattern, footprint from sub-period to multi-period, directions over
+the hemisphere).  The recipe and draw order are documented in DESIGN.md "Input recipe".
+
+Served to both the oracle (via tests/bench) and the CUDA path; imports neither.
+Everything is numpy; one ``numpy.random.default_rng(seed)`` per config, fixed draw order.
+"""
+import math
+
+import numpy as np
+
+QUERY_DTYPE = np.dtype([("u", "<f4"), ("v", "<f4"), ("footprint", "<f4"), ("material", "<i4"),
+                        ("wi", "<f4", (3,)), ("wo", "<f4", (3,))], align=False)
+LIGHT_DTYPE = np.dtype([("type", "<i4"), ("vec", "<f4", (3,)), ("rgb", "<f4", (3,)),
+                        ("emit_n", "<f4", (3,))], align=False)
+FEAT_DIM = 32
+
+
+def round_to_bf16(a):
+    """fp32 -> nearest bf16-representable fp32 (round to nearest even on the dropped 16 bits).
+    'Weights stored in bf16' (BASELINE.json configs[1]): the stored values ARE the model, and both
+    the oracle and the CUDA library are handed these already-rounded fp32 arrays."""
+    x = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    lsb = (x >> 16) & 1
+    r = ((x + 0x7FFF + lsb) >> 16) << 16
+    return r.astype(np.uint32).view(np.float32).reshape(np.shape(a))
+
+
+def layer_shapes(L, H, F=FEAT_DIM):
+    return [(H, L + 3), (H, H), (F, H), (H, F + 6), (H, H), (3, H)]
+
+
+def make_network(rng, L=16, H=64, F=FEAT_DIM, bf16_weights=False):
+    """Xavier-uniform weights (gain 1), biases 0.01*N(0,1), fp32.  Draw order: W1,b1,...,W6,b6."""
+    Ws, bs = [], []
+    for (n_out, n_in) in layer_shapes(L, H, F):
+        a = math.sqrt(6.0 / (n_in + n_out))
+        W = rng.uniform(-a, a, size=(n_out, n_in)).astype(np.float32)
+        b = (0.01 * rng.standard_normal(n_out)).astype(np.float32)
+        Ws.append(round_to_bf16(W) if bf16_weights else W)
+        bs.append(b)
+    return Ws, bs
+
+
+def make_latents(rng, M, L):
+    return rng.standard_normal((M, L)).astype(np.float32)
+
+
+def cosine_hemisphere(rng, n):
+    """r = sqrt(xi1), phi = 2 pi xi2, w = (r cos phi, r sin phi, sqrt(1 - xi1))."""
+    xi1 = rng.random(n)
+    xi2 = rng.random(n)
+    r = np.sqrt(xi1)
+    phi = 2.0 * np.pi * xi2
+    return np.stack([r * np.cos(phi), r * np.sin(phi), np.sqrt(1.0 - xi1)], axis=1).astype(np.float32)
+
+
+def make_queries(rng, n, M):
+    """Draw order: u, v, log2 fp, wi, wo, material."""
+    q = np.zeros(n, dtype=QUERY_DTYPE)
+    q["u"] = rng.random(n).astype(np.float32)
+    q["v"] = rng.random(n).astype(np.float32)
+    q["footprint"] = np.exp2(rng.uniform(-8.0, 0.0, n)).astype(np.float32)
+    q["wi"] = cosine_hemisphere(rng, n)
+    q["wo"] = cosine_hemisphere(rng, n)
+    q["material"] = rng.integers(0, M, n).astype(np.int32) if M > 1 else 0
+    return q
+
+
+def make_frames(rng, n):
+    """Per-query world frames [n][6] = (n, t): random unit normal, random non-parallel tangent hint."""
+    nrm = rng.standard_normal((n, 3))
+    nrm /= np.linalg.norm(nrm, axis=1, keepdims=True)
+    tan = rng.standard_normal((n, 3))
+    return np.concatenate([nrm, tan], axis=1).astype(np.float32)
+
+
+def make_gbuffer(rng, width, height, uv_scale=12.0, n_ids=8, tile=64):
+    """Plane z=0 seen by a pinhole at (0,0,1) looking -z, vertical FOV 60 deg, ray through (px+1/2, py+1/2).
+    uv = uv_scale * ((px+1/2)/W, (py+1/2)/H) (left unwrapped -- the library wraps);
+    footprint = max(|duv/dx|, |duv/dy|) = uv_scale / H (analytic screen-space derivative);
+    normal tilted a ~ U[0, 30 deg] about +z at azimuth phi ~ U[0, 2 pi); tangent hint (1,0,0);
+    material = ((px>>6) + (py>>6)) mod n_ids.  Draw order: a, phi."""
+    W, H = int(width), int(height)
+    px = (np.arange(W, dtype=np.float64) + 0.5)[None, :].repeat(H, 0)
+    py = (np.arange(H, dtype=np.float64) + 0.5)[:, None].repeat(W, 1)
+    th = math.tan(math.radians(30.0))
+    x = (2.0 * px / W - 1.0) * (W / H) * th
+    y = (1.0 - 2.0 * py / H) * th
+    npx = W * H
+    a = rng.uniform(0.0, math.radians(30.0), npx)
+    phi = rng.uniform(0.0, 2.0 * np.pi, npx)
+    pos_fp = np.empty((npx, 4), np.float32)
+    pos_fp[:, 0] = x.reshape(-1)
+    pos_fp[:, 1] = y.reshape(-1)
+    pos_fp[:, 2] = 0.0
+    pos_fp[:, 3] = max(uv_scale / W, uv_scale / H)
+    nrm_u = np.empty((npx, 4), np.float32)
+    nrm_u[:, 0] = np.sin(a) * np.cos(phi)
+    nrm_u[:, 1] = np.sin(a) * np.sin(phi)
+    nrm_u[:, 2] = np.cos(a)
+    nrm_u[:, 3] = (uv_scale * px / W).reshape(-1)
+    tan_v = np.empty((npx, 4), np.float32)
+    tan_v[:, 0] = 1.0
+    tan_v[:, 1] = 0.0
+    tan_v[:, 2] = 0.0
+    tan_v[:, 3] = (uv_scale * py / H).reshape(-1)
+    ix = (np.arange(W) // tile)[None, :]
+    iy = (np.arange(H) // tile)[:, None]
+    material = ((ix + iy) % n_ids).astype(np.int32).reshape(-1)
+    return {"pos_fp": pos_fp, "nrm_u": nrm_u, "tan_v": tan_v, "material": material,
+            "width": W, "height": H, "cam_pos": np.array([0.0, 0.0, 1.0], np.float32)}
+
+
+def lights_direct5():
+    """configs[2]: 1 directional light toward (0.3,0.2,1)/|.| with radiance (1,1,1), plus 4 point
+    lights at (+-0.6, +-0.35, 0.5) with distinct RGB intensities ~0.5."""
+    lt = np.zeros(5, dtype=LIGHT_DTYPE)
+    d = np.array([0.3, 0.2, 1.0])
+    lt[0]["type"] = 0
+    lt[0]["vec"] = (d / np.linalg.norm(d)).astype(np.float32)
+    lt[0]["rgb"] = (1.0, 1.0, 1.0)
+    inten = [(0.6, 0.5, 0.4), (0.4, 0.5, 0.6), (0.5, 0.6, 0.4), (0.5, 0.4, 0.6)]
+    k = 1
+    for sx in (-1.0, 1.0):
+        for sy in (-1.0, 1.0):
+            lt[k]["type"] = 1
+            lt[k]["vec"] = (0.6 * sx, 0.35 * sy, 0.5)
+            lt[k]["rgb"] = inten[k - 1]
+            k += 1
+    return lt
+
+
+def lights_area16(rng, side=0.5, z=0.8, Le=8.0):
+    """configs[3]: one side x side emitter at height z facing -z, sampled at 4x4 jittered strata and
+    passed as 16 point lights with rgb = Le*A/16 and emit_n = (0,0,-1); the same 16 samples serve
+    every pixel (no RNG inside either implementation).  Draw order: jitter x (16), jitter y (16)."""
+    jx = rng.random(16)
+    jy = rng.random(16)
+    lt = np.zeros(16, dtype=LIGHT_DTYPE)
+    for s in range(16):
+        i, j = s % 4, s // 4
+        lt[s]["type"] = 1
+        lt[s]["vec"] = ((-0.5 + (i + jx[s]) / 4.0) * side, (-0.5 + (j + jy[s]) / 4.0) * side, z)
+        lt[s]["rgb"] = (Le * side * side / 16.0,) * 3
+        lt[s]["emit_n"] = (0.0, 0.0, -1.0)
+    return lt
+
+
+def sweep_seed(i_n, i_h, i_l):
+    return 1000 + 9 * i_n + 3 * i_h + i_l
+
+
+def config(idx, n=None, width=None, height=None, L=16, H=64, seed=None):
+    """The five BASELINE.json configs as dicts of numpy arrays.  seed defaults to the config index."""
+    rng = np.random.default_rng(idx if seed is None else seed)
+    if idx == 0:
+        Ws, bs = make_network(rng, L, H)
+        Z = make_latents(rng, 1, L)
+        q = make_queries(rng, 4096 if n is None else n, 1)
+        return {"name": "tiny_eval", "weights": Ws, "biases": bs, "latents": Z, "queries": q}
+    if idx in (1, 4):
+        Ws, bs = make_network(rng, L, H, bf16_weights=True)
+        Z = make_latents(rng, 8, L)
+        q = make_queries(rng, (1 << 20) if n is None else n, 8)
+        return {"name": "batch_eval" if idx == 1 else "sweep_point", "weights": Ws, "biases": bs,
+                "latents": Z, "queries": q}
+    if idx == 2:
+        Ws, bs = make_network(rng, L, H, bf16_weights=True)
+        Z = make_latents(rng, 8, L)
+        g = make_gbuffer(rng, 1920 if width is None else width, 1080 if height is None else height)
+        return {"name": "frame_1080p_5lights", "weights": Ws, "biases": bs, "latents": Z, "gbuffer": g,
+                "lights": lights_direct5()}
+    if idx == 3:
+        Ws, bs = make_network(rng, L, H, bf16_weights=True)
+        Z = make_latents(rng, 8, L)
+        g = make_gbuffer(rng, 3840 if width is None else width, 2160 if height is None else height)
+        lights = lights_area16(rng)
+        z_edit = rng.standard_normal(L).astype(np.float32)
+        return {"name": "frame_4k_16lights_edit", "weights": Ws, "biases": bs, "latents": Z, "gbuffer": g,
+                "lights": lights, "edit_material": 3, "edit_latent": z_edit}
+    raise ValueError(idx)

@@ -1,0 +1,142 @@
+/*
+ * nbsdf.h -- C ABI of libnbsdf.so: the B200 (sm_100a) neural woven-fabric BSDF decoder.
+ *
+ * The calls follow the problem statement of "Real-time Neural Woven Fabric Rendering"
+ * (arXiv 2406.17782; citations are /root/reference/PAPER.md line numbers):
+ *   decoder signature (z, position, size, wi, wo) -> BSDF value ......... PAPER.md:160, Eq. 7 at 149
+ *   two-MLP decoder (spatial fusion MLP-A, angular decoder MLP-B) ....... PAPER.md:164 (sec. 4.2 "Decoder")
+ *   per-frame recipe (query + lighting -> decoder -> BSDF x lighting) ... PAPER.md:196 (sec. 4.3 "Rendering")
+ *   editing = replace the material latent vector between frames ......... PAPER.md:198 (sec. 4.3 "Editing")
+ * The network shapes are those of BASELINE.json configs (DESIGN.md "Readings" #1):
+ *   MLP-A: [z(L), u', v', log2 fp] -> H (ReLU) -> H (ReLU) -> F (linear feature), F = 32
+ *   MLP-B: [feat(F), wi(3), wo(3)] -> H (ReLU) -> H (ReLU) -> 3, softplus
+ *
+ * Conventions
+ *   - All pointers are plain C pointers; each parameter says whether it is HOST or DEVICE memory.
+ *   - The caller owns every query / G-buffer / output buffer and the CUDA stream (passed as void* =
+ *     cudaStream_t; NULL = the legacy default stream).  The library owns only its packed weights,
+ *     latent table and light staging, all released by nbsdf_destroy.  HOST arrays handed to
+ *     nbsdf_create / nbsdf_set_latents / nbsdf_shade_frame(lights) are copied before the call returns.
+ *   - nbsdf_eval / nbsdf_shade_frame / nbsdf_set_latents only enqueue work on the given stream and
+ *     return; there is no internal synchronisation.  Work is ordered by the stream: a set_latents is
+ *     visible to every later launch on the same stream (the editing guarantee of PAPER.md:198).
+ *   - Every call returns an nbsdf_status and never throws or aborts; nbsdf_last_error gives text.
+ *     On NBSDF_E_INVALID nothing is launched.  There is no CPU fallback: a device that is not
+ *     sm_100 makes nbsdf_create fail with NBSDF_E_UNSUPPORTED.
+ *   - Directions are unit length; wi points from the surface to the light, wo to the viewer.  Without a
+ *     frame they are already local (+z = macro normal).  material in [0, max_materials); a negative
+ *     material yields exactly (0,0,0); material >= max_materials is undefined behaviour.
+ *     Inputs must be finite.
+ */
+#ifndef NBSDF_H
+#define NBSDF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nbsdf_ctx nbsdf_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    NBSDF_OK = 0,
+    NBSDF_E_INVALID = -1,     /* NULL pointer, negative size, misaligned buffer, range error */
+    NBSDF_E_UNSUPPORTED = -2, /* device is not sm_100, or dims outside the supported set */
+    NBSDF_E_CUDA = -3,        /* a CUDA runtime call failed; see nbsdf_last_error */
+    NBSDF_E_NOMEM = -4
+} nbsdf_status;
+
+typedef enum {
+    NBSDF_PREC_FP32 = 0, /* CUDA-core variant: fp32 FMA everywhere (no TF32, no tensor cores); <= 1e-5 vs oracle */
+    NBSDF_PREC_BF16 = 1, /* tcgen05 tensor cores, bf16 operands, fp32 accumulate in TMEM */
+    NBSDF_PREC_FP16 = 2  /* tcgen05 tensor cores, fp16 operands (bf16-stored weights convert exactly), fp32 accumulate */
+} nbsdf_precision;
+
+/* Supported: latent_dim in {8,16,32}, hidden in {32,64,128}, feat_dim == 32, 1 <= max_materials <= 64. */
+typedef struct {
+    int32_t latent_dim;    /* L */
+    int32_t hidden;        /* H */
+    int32_t feat_dim;      /* F */
+    int32_t max_materials; /* M: rows of the latent table */
+    int32_t precision;     /* nbsdf_precision */
+    int32_t device;        /* CUDA device ordinal */
+} nbsdf_config;
+
+/* HOST pointers, fp32, row-major W[k][out][in], y = W x + b.  Layer input widths:
+ * W[0]: H x (L+3), W[1]: H x H, W[2]: F x H, W[3]: H x (F+6), W[4]: H x H, W[5]: 3 x H.
+ * In the tensor-core precisions the weights are rounded to the operand type (RNE) at create; biases,
+ * latents, queries and outputs stay fp32. */
+typedef struct {
+    const float* W[6];
+    const float* b[6];
+} nbsdf_weights;
+
+/* One shading query, 40 bytes, array-of-structs (position, size, wi, wo + material). */
+typedef struct {
+    float u, v;       /* footprint position in pattern units; wrapped to [0,1) by the library */
+    float footprint;  /* footprint side length in pattern units; log2 of clamp(., 2^-20, 2^4) is fed to MLP-A */
+    int32_t material; /* row of the latent table; < 0 => output (0,0,0) */
+    float wi[3];      /* to the light */
+    float wo[3];      /* to the viewer */
+} nbsdf_query;
+
+/* Headless G-buffer, DEVICE planes, 52 bytes per pixel; pixel index = y * width + x. */
+typedef struct {
+    const float* pos_fp;     /* [h*w][4]: world x, y, z, footprint   (16-byte aligned) */
+    const float* nrm_u;      /* [h*w][4]: shading normal nx, ny, nz, u               */
+    const float* tan_v;      /* [h*w][4]: tangent hint tx, ty, tz, v                 */
+    const int32_t* material; /* [h*w]; < 0 = background => radiance (0,0,0)          */
+    int32_t width, height;
+    float cam_pos[3];        /* pinhole position; wo = normalize(cam_pos - x)        */
+} nbsdf_gbuffer;
+
+/* type 0: directional, vec = direction TO the light (normalised by the library), rgb = radiance E.
+ * type 1: point, vec = position, rgb = intensity I;  E = I * max(0, -wi . emit_n) / |vec - x|^2,
+ *         emit_n = (0,0,0) => isotropic (factor 1). */
+typedef struct {
+    int32_t type;
+    float vec[3];
+    float rgb[3];
+    float emit_n[3];
+} nbsdf_light;
+
+#define NBSDF_MAX_LIGHTS 32
+
+/* Builds a decoder context on cfg->device: validates dims, packs the weights for the chosen precision
+ * (tensor-core paths: operand type, K padded to 16, 128-byte-swizzled K-major tiles as tcgen05 reads them),
+ * allocates the latent table (zero-filled).  weights: HOST, copied.  *out receives the context. */
+int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weights, nbsdf_ctx** out);
+
+/* Overwrites rows [first, first+count) of the material latent table ("update the material
+ * latent vector").  latents_host: HOST, count x L fp32, copied before return; the device update is enqueued
+ * on cuda_stream and ordered before later launches on it.  first+count > max_materials => NBSDF_E_INVALID. */
+int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, const float* latents_host, void* cuda_stream);
+
+/* Batched decoder inference: stages A1-A4, B1-B7 of DESIGN.md in one fused kernel.
+ * q_dev: DEVICE, n records, 16-byte aligned.  frames_dev: DEVICE [n][6] = (normal, tangent hint) per query in
+ * the space of wi/wo, or NULL when wi/wo are already local.  rgb_dev: DEVICE [n][3] fp32, 16-byte aligned.
+ * n == 0 is a no-op returning NBSDF_OK. */
+int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float* frames_dev, int64_t n, float* rgb_dev,
+               void* cuda_stream);
+
+/* Frame shading: per pixel, MLP-A once, MLP-B once per light,
+ * radiance[p] = sum_l rgb(z_m, uv, fp, wi_l, wo) * E_l * max(0, wi_l,local.z), lights in index order.
+ * gbuf: HOST struct holding DEVICE plane pointers.  lights_host: HOST, n_lights <= NBSDF_MAX_LIGHTS, copied.
+ * radiance_dev: DEVICE [h][w][3] fp32, 16-byte aligned. */
+int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* gbuf, const nbsdf_light* lights_host, int32_t n_lights,
+                      float* radiance_dev, void* cuda_stream);
+
+/* Frees everything the context owns.  The caller must have synchronised the streams it used.  NULL is allowed. */
+void nbsdf_destroy(nbsdf_ctx* ctx);
+
+/* Text of the last error on this context (or of the last failed nbsdf_create when ctx == NULL).  Never NULL. */
+const char* nbsdf_last_error(const nbsdf_ctx* ctx);
+
+/* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
+int64_t nbsdf_launch_count(const nbsdf_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBSDF_H */

@@ -1,0 +1,169 @@
+// nbsdf_common.cuh -- shared declarations of the CUDA library (host context + kernel parameter blocks)
+// and the per-query input assembly (stages A2-A4, C1 of DESIGN.md).  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/nbsdf.h"
+
+namespace nbsdf {
+
+constexpr int kFeat = 32;          // F: feature width of MLP-A (BASELINE.json configs[0])
+constexpr int kTileRows = 128;     // queries per tile = TMEM lanes = threads per warpgroup
+
+// Device pointers + dims handed to every kernel (by value).
+struct NetParams {
+    const float* latents;   // [M][L] fp32 latent table ("material latent vector")
+    const float* w32;       // fp32 path: transposed, padded weights + biases (see pack_fp32)
+    const uint8_t* wimg;    // tensor path: shared-memory image (weights as swizzled UMMA tiles, biases)
+    int32_t L, H, M;
+    uint32_t wimg_bytes;
+};
+
+struct LightParams {
+    nbsdf_light light[NBSDF_MAX_LIGHTS];   // directional vec already normalised on the host
+    int32_t n;
+};
+
+struct FrameParams {
+    const float4* pos_fp;
+    const float4* nrm_u;
+    const float4* tan_v;
+    const int32_t* material;
+    int64_t n_pixels;
+    float cam[3];
+};
+
+// ---------------------------------------------------------------------------------------------
+// Stage A2: wrap to the pattern period (period 1).  floor-based, so negatives land in [0,1].
+__device__ __forceinline__ float wrap01(float x) { return x - floorf(x); }
+
+// Stage A3: log2 of the footprint clamped to [2^-20, 2^4].  fmaxf/fminf also turn fp <= 0 (and NaN) into the bound.
+template <bool kFast>
+__device__ __forceinline__ float log_footprint(float fp)
+{
+    float c = fminf(fmaxf(fp, 9.5367431640625e-07f), 16.0f);
+    return kFast ? __log2f(c) : log2f(c);
+}
+
+struct Frame {
+    float t[3], b[3], n[3];
+};
+
+// Stage A4: orthonormal frame from (n, tangent hint): n^ = n/|n|, t' = t - n^(n^.t), degenerate t' replaced by
+// e_k - n^ n^_k with k = argmin |n^_k| (lowest k on ties), b^ = n^ x t^.
+__device__ __forceinline__ Frame make_frame(float nx, float ny, float nz, float tx, float ty, float tz)
+{
+    Frame f;
+    float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
+    nx *= inv; ny *= inv; nz *= inv;
+    float nt = nx * tx + ny * ty + nz * tz;
+    tx -= nx * nt; ty -= ny * nt; tz -= nz * nt;
+    float tt = tx * tx + ty * ty + tz * tz;
+    if (tt < 1e-12f) {
+        float ax = fabsf(nx), ay = fabsf(ny), az = fabsf(nz);
+        int k = 0;
+        float am = ax;
+        if (ay < am) { k = 1; am = ay; }
+        if (az < am) { k = 2; }
+        float nk = k == 0 ? nx : (k == 1 ? ny : nz);
+        tx = (k == 0 ? 1.0f : 0.0f) - nx * nk;
+        ty = (k == 1 ? 1.0f : 0.0f) - ny * nk;
+        tz = (k == 2 ? 1.0f : 0.0f) - nz * nk;
+        tt = tx * tx + ty * ty + tz * tz;
+    }
+    inv = rsqrtf(tt);
+    tx *= inv; ty *= inv; tz *= inv;
+    f.n[0] = nx; f.n[1] = ny; f.n[2] = nz;
+    f.t[0] = tx; f.t[1] = ty; f.t[2] = tz;
+    f.b[0] = ny * tz - nz * ty;
+    f.b[1] = nz * tx - nx * tz;
+    f.b[2] = nx * ty - ny * tx;
+    return f;
+}
+
+__device__ __forceinline__ void to_local(const Frame& f, float x, float y, float z, float out[3])
+{
+    out[0] = x * f.t[0] + y * f.t[1] + z * f.t[2];
+    out[1] = x * f.b[0] + y * f.b[1] + z * f.b[2];
+    out[2] = x * f.n[0] + y * f.n[1] + z * f.n[2];
+}
+
+// Stage C1: direction to light l and its irradiance factor E at world position x.
+__device__ __forceinline__ void light_sample(const nbsdf_light& lt, float px, float py, float pz, float wi[3], float E[3])
+{
+    if (lt.type == 0) {
+        wi[0] = lt.vec[0]; wi[1] = lt.vec[1]; wi[2] = lt.vec[2];
+        E[0] = lt.rgb[0]; E[1] = lt.rgb[1]; E[2] = lt.rgb[2];
+    } else {
+        float vx = lt.vec[0] - px, vy = lt.vec[1] - py, vz = lt.vec[2] - pz;
+        float d2 = vx * vx + vy * vy + vz * vz;
+        float inv = rsqrtf(d2);
+        wi[0] = vx * inv; wi[1] = vy * inv; wi[2] = vz * inv;
+        float fac = 1.0f;
+        if (lt.emit_n[0] != 0.0f || lt.emit_n[1] != 0.0f || lt.emit_n[2] != 0.0f)
+            fac = fmaxf(0.0f, -(wi[0] * lt.emit_n[0] + wi[1] * lt.emit_n[1] + wi[2] * lt.emit_n[2]));
+        float s = fac * inv * inv;
+        E[0] = lt.rgb[0] * s; E[1] = lt.rgb[1] * s; E[2] = lt.rgb[2] * s;
+    }
+}
+
+// Stage B7: softplus(x) = ln(1 + e^x), beta = 1, no threshold.
+template <bool kFast>
+__device__ __forceinline__ float softplus(float x)
+{
+    if (kFast) {
+        float t = __expf(-fabsf(x));
+        // log1p(t): series below 0.01 keeps the tail (x << 0) relatively accurate, MUFU.LG2 above
+        float l = t < 0.01f ? t * (1.0f - t * (0.5f - t * 0.33333334f)) : __logf(1.0f + t);
+        return fmaxf(x, 0.0f) + l;
+    }
+    return x > 0.0f ? x + log1pf(expf(-x)) : log1pf(expf(x));
+}
+
+// ---------------------------------------------------------------------------------------------
+// launchers implemented in nbsdf_fp32.cu / nbsdf_tc.cu; return the cudaError_t of the launch
+cudaError_t launch_eval_fp32(const NetParams& net, const nbsdf_query* q, const float* frames, int64_t n, float* rgb,
+                             cudaStream_t s);
+cudaError_t launch_shade_fp32(const NetParams& net, const FrameParams& fr, const LightParams& lights, float* out,
+                              cudaStream_t s);
+cudaError_t launch_eval_tc(const NetParams& net, int precision, int num_sms, const nbsdf_query* q, const float* frames,
+                           int64_t n, float* rgb, cudaStream_t s);
+cudaError_t launch_shade_tc(const NetParams& net, int precision, int num_sms, const FrameParams& fr,
+                            const LightParams& lights, float* out, cudaStream_t s);
+cudaError_t init_tc(int L, int H);       // cudaFuncSetAttribute for the instantiations in use
+cudaError_t init_fp32();
+
+// shared-memory image layout of the tensor path, computed identically on host (packing) and device (carving)
+struct TcLayout {
+    int K1p, K4p;            // padded K of layers 1 and 4 (multiples of 16)
+    uint32_t w_off[6];       // byte offset of each layer's weight tiles (1024-aligned)
+    uint32_t w_rows[6];      // padded N (rows) of each layer
+    uint32_t bias_off[6];    // byte offset of each layer's fp32 biases
+    uint32_t total;          // bytes of the image (multiple of 16)
+};
+
+__host__ __device__ inline int pad16(int k) { return (k + 15) & ~15; }
+
+__host__ __device__ inline TcLayout tc_layout(int L, int H)
+{
+    TcLayout t;
+    t.K1p = pad16(L + 3);
+    t.K4p = pad16(kFeat + 6);
+    const int K[6] = { t.K1p, H, H, t.K4p, H, H };
+    const int N[6] = { H, H, kFeat, H, H, 16 };
+    uint32_t off = 0;
+    for (int l = 0; l < 6; ++l) {
+        t.w_off[l] = off;
+        t.w_rows[l] = (uint32_t)N[l];
+        off += (uint32_t)((K[l] + 63) / 64) * (uint32_t)N[l] * 128u;   // N rows x 128 B per 64-wide K block
+    }
+    for (int l = 0; l < 6; ++l) {
+        t.bias_off[l] = off;
+        off += (uint32_t)N[l] * 4u;
+    }
+    t.total = (off + 15u) & ~15u;
+    return t;
+}
+
+}  // namespace nbsdf

@@ -1,0 +1,277 @@
+// nbsdf_host.cu -- the C ABI of include/nbsdf.h: context, weight packing, latent table, launches.
+// No CPU fallback anywhere: every compute call ends in a kernel launch or an error code.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "nbsdf_common.cuh"
+
+namespace nbsdf {
+void pack_fp32(int L, int H, const nbsdf_weights* w, float* blob);
+size_t fp32_blob_floats(int L, int H);
+}  // namespace nbsdf
+
+using namespace nbsdf;
+
+struct nbsdf_ctx {
+    nbsdf_config cfg;
+    int num_sms = 0;
+    float* d_latents = nullptr;       // [M][L] fp32
+    float* d_w32 = nullptr;           // fp32 path blob
+    uint8_t* d_wimg = nullptr;        // tensor path shared-memory image
+    uint32_t wimg_bytes = 0;
+    float* h_stage = nullptr;         // pinned mirror used by set_latents
+    cudaEvent_t stage_free = nullptr; // recorded after the last staged copy
+    bool stage_busy = false;
+    int64_t launches = 0;
+    std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(nbsdf_ctx* ctx, int code, const std::string& msg)
+{
+    if (ctx) ctx->err = msg; else g_create_err = msg;
+    return code;
+}
+
+static int fail_cuda(nbsdf_ctx* ctx, const char* what, cudaError_t e)
+{
+    return fail(ctx, NBSDF_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+// fp32 -> operand type bits, round to nearest even
+static uint16_t to_op16(float v, bool bf16)
+{
+    if (bf16) return __bfloat16_as_ushort(__float2bfloat16_rn(v));
+    return __half_as_ushort(__float2half_rn(v));
+}
+
+// Shared-memory image of the tensor path: per layer, per 64-wide K block, N rows of 128 bytes, K-major, with the
+// 16-byte chunk index XOR-ed by (row % 8) (the 128-byte swizzle tcgen05 applies when it reads the tile), then biases.
+static void pack_tc(int L, int H, bool bf16, const nbsdf_weights* w, uint8_t* img)
+{
+    const TcLayout lay = tc_layout(L, H);
+    const int Kr[6] = { L + 3, H, H, kFeat + 6, H, H };
+    const int Kp[6] = { lay.K1p, H, H, lay.K4p, H, H };
+    const int Nr[6] = { H, H, kFeat, H, H, 3 };
+    memset(img, 0, lay.total);
+    for (int l = 0; l < 6; ++l) {
+        const int Np = (int)lay.w_rows[l];
+        for (int n = 0; n < Nr[l]; ++n) {
+            for (int k = 0; k < Kr[l]; ++k) {
+                const int kb = k / 64, kk = k % 64;
+                const int chunk = (kk / 8) ^ (n % 8);
+                const size_t off = lay.w_off[l] + (size_t)kb * Np * 128 + (size_t)n * 128 + (size_t)chunk * 16 + (size_t)(kk % 8) * 2;
+                const uint16_t bits = to_op16(w->W[l][(size_t)n * Kr[l] + k], bf16);
+                memcpy(img + off, &bits, 2);
+            }
+            memcpy(img + lay.bias_off[l] + (size_t)n * 4, &w->b[l][n], 4);
+        }
+        (void)Kp;
+    }
+}
+
+static bool dims_supported(const nbsdf_config* c)
+{
+    const bool l_ok = c->latent_dim == 8 || c->latent_dim == 16 || c->latent_dim == 32;
+    const bool h_ok = c->hidden == 32 || c->hidden == 64 || c->hidden == 128;
+    return l_ok && h_ok && c->feat_dim == kFeat && c->max_materials >= 1 && c->max_materials <= 64;
+}
+
+extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weights, nbsdf_ctx** out)
+{
+    if (!cfg || !weights || !out) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create: NULL argument");
+    *out = nullptr;
+    for (int l = 0; l < 6; ++l)
+        if (!weights->W[l] || !weights->b[l]) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create: NULL weight or bias pointer");
+    if (cfg->precision < NBSDF_PREC_FP32 || cfg->precision > NBSDF_PREC_FP16)
+        return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create: unknown precision");
+    if (!dims_supported(cfg))
+        return fail(nullptr, NBSDF_E_UNSUPPORTED,
+                    "nbsdf_create: supported dims are latent_dim in {8,16,32}, hidden in {32,64,128}, feat_dim 32, 1..64 materials");
+    int n_dev = 0;
+    cudaError_t e = cudaGetDeviceCount(&n_dev);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceCount", e);
+    if (cfg->device < 0 || cfg->device >= n_dev) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create: no such device");
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, cfg->device);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceProperties", e);
+    if (prop.major != 10)
+        return fail(nullptr, NBSDF_E_UNSUPPORTED, "nbsdf_create: device is not sm_100 (Blackwell B200); there is no fallback path");
+    e = cudaSetDevice(cfg->device);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaSetDevice", e);
+
+    nbsdf_ctx* ctx = new (std::nothrow) nbsdf_ctx();
+    if (!ctx) return fail(nullptr, NBSDF_E_NOMEM, "nbsdf_create: out of host memory");
+    ctx->cfg = *cfg;
+    ctx->num_sms = prop.multiProcessorCount;
+    const int L = cfg->latent_dim, H = cfg->hidden, M = cfg->max_materials;
+
+#define NBSDF_TRY(call, what)                                                    \
+    do {                                                                         \
+        cudaError_t e_ = (call);                                                 \
+        if (e_ != cudaSuccess) {                                                 \
+            int rc_ = fail_cuda(nullptr, what, e_);                              \
+            nbsdf_destroy(ctx);                                                  \
+            return e_ == cudaErrorMemoryAllocation ? NBSDF_E_NOMEM : rc_;        \
+        }                                                                        \
+    } while (0)
+
+    NBSDF_TRY(cudaMalloc(&ctx->d_latents, (size_t)M * L * sizeof(float)), "cudaMalloc(latents)");
+    NBSDF_TRY(cudaMemset(ctx->d_latents, 0, (size_t)M * L * sizeof(float)), "cudaMemset(latents)");
+    NBSDF_TRY(cudaMallocHost(&ctx->h_stage, (size_t)M * L * sizeof(float)), "cudaMallocHost(stage)");
+    NBSDF_TRY(cudaEventCreateWithFlags(&ctx->stage_free, cudaEventDisableTiming), "cudaEventCreate");
+    if (cfg->precision == NBSDF_PREC_FP32) {
+        std::vector<float> blob(fp32_blob_floats(L, H));
+        pack_fp32(L, H, weights, blob.data());
+        NBSDF_TRY(cudaMalloc(&ctx->d_w32, blob.size() * sizeof(float)), "cudaMalloc(w32)");
+        NBSDF_TRY(cudaMemcpy(ctx->d_w32, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(w32)");
+        NBSDF_TRY(init_fp32(), "cudaFuncSetAttribute(fp32)");
+    } else {
+        const TcLayout lay = tc_layout(L, H);
+        std::vector<uint8_t> img(lay.total);
+        pack_tc(L, H, cfg->precision == NBSDF_PREC_BF16, weights, img.data());
+        ctx->wimg_bytes = lay.total;
+        NBSDF_TRY(cudaMalloc(&ctx->d_wimg, lay.total), "cudaMalloc(wimg)");
+        NBSDF_TRY(cudaMemcpy(ctx->d_wimg, img.data(), lay.total, cudaMemcpyHostToDevice), "cudaMemcpy(wimg)");
+        NBSDF_TRY(init_tc(L, H), "cudaFuncSetAttribute(tc)");
+    }
+#undef NBSDF_TRY
+    *out = ctx;
+    return NBSDF_OK;
+}
+
+extern "C" void nbsdf_destroy(nbsdf_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->stage_busy && ctx->stage_free) cudaEventSynchronize(ctx->stage_free);
+    if (ctx->d_latents) cudaFree(ctx->d_latents);
+    if (ctx->d_w32) cudaFree(ctx->d_w32);
+    if (ctx->d_wimg) cudaFree(ctx->d_wimg);
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->stage_free) cudaEventDestroy(ctx->stage_free);
+    delete ctx;
+}
+
+extern "C" const char* nbsdf_last_error(const nbsdf_ctx* ctx)
+{
+    return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+extern "C" int64_t nbsdf_launch_count(const nbsdf_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, const float* latents_host, void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (first < 0 || count < 0 || (int64_t)first + count > ctx->cfg.max_materials)
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_latents: rows out of range");
+    if (count == 0) return NBSDF_OK;
+    if (!latents_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_latents: NULL latents");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int L = ctx->cfg.latent_dim;
+    cudaError_t e = cudaSetDevice(ctx->cfg.device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    // the pinned mirror may still be the source of an earlier in-flight copy: wait for that copy only
+    if (ctx->stage_busy) {
+        e = cudaEventSynchronize(ctx->stage_free);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventSynchronize", e);
+        ctx->stage_busy = false;
+    }
+    float* src = ctx->h_stage + (size_t)first * L;
+    memcpy(src, latents_host, (size_t)count * L * sizeof(float));
+    e = cudaMemcpyAsync(ctx->d_latents + (size_t)first * L, src, (size_t)count * L * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemcpyAsync(latents)", e);
+    e = cudaEventRecord(ctx->stage_free, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
+    ctx->stage_busy = true;
+    return NBSDF_OK;
+}
+
+static NetParams net_params(const nbsdf_ctx* ctx)
+{
+    NetParams p;
+    p.latents = ctx->d_latents;
+    p.w32 = ctx->d_w32;
+    p.wimg = ctx->d_wimg;
+    p.L = ctx->cfg.latent_dim;
+    p.H = ctx->cfg.hidden;
+    p.M = ctx->cfg.max_materials;
+    p.wimg_bytes = ctx->wimg_bytes;
+    return p;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+extern "C" int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float* frames_dev, int64_t n, float* rgb_dev,
+                          void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (n < 0) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: negative n");
+    if (n == 0) return NBSDF_OK;
+    if (!q_dev || !rgb_dev) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: NULL buffer");
+    if (!aligned16(q_dev) || !aligned16(rgb_dev) || (frames_dev && (reinterpret_cast<uintptr_t>(frames_dev) & 7u)))
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: queries/outputs must be 16-byte aligned, frames 8-byte aligned");
+    cudaError_t e = cudaSetDevice(ctx->cfg.device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    const NetParams net = net_params(ctx);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_eval_fp32(net, q_dev, frames_dev, n, rgb_dev, s);
+    else e = launch_eval_tc(net, ctx->cfg.precision, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_eval launch", e);
+    ctx->launches += 1;
+    return NBSDF_OK;
+}
+
+extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const nbsdf_light* lights_host, int32_t n_lights,
+                                 float* radiance_dev, void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (!g) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL gbuffer");
+    if (g->width < 0 || g->height < 0) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: negative size");
+    if (n_lights < 0 || n_lights > NBSDF_MAX_LIGHTS) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: n_lights must be in [0, 32]");
+    if (n_lights > 0 && !lights_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL lights");
+    const int64_t npx = (int64_t)g->width * g->height;
+    if (npx == 0) return NBSDF_OK;
+    if (!g->pos_fp || !g->nrm_u || !g->tan_v || !g->material || !radiance_dev)
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL buffer");
+    if (!aligned16(g->pos_fp) || !aligned16(g->nrm_u) || !aligned16(g->tan_v) || !aligned16(radiance_dev))
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: planes and output must be 16-byte aligned");
+    for (int l = 0; l < n_lights; ++l)
+        if (lights_host[l].type != 0 && lights_host[l].type != 1)
+            return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: light type must be 0 (directional) or 1 (point)");
+    cudaError_t e = cudaSetDevice(ctx->cfg.device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+
+    LightParams lp;
+    memset(&lp, 0, sizeof lp);
+    lp.n = n_lights;
+    for (int l = 0; l < n_lights; ++l) {
+        lp.light[l] = lights_host[l];
+        if (lp.light[l].type == 0) {   // normalise the direction once, in double
+            const double x = lp.light[l].vec[0], y = lp.light[l].vec[1], z = lp.light[l].vec[2];
+            const double len = sqrt(x * x + y * y + z * z);
+            if (!(len > 0.0)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: zero-length light direction");
+            lp.light[l].vec[0] = (float)(x / len); lp.light[l].vec[1] = (float)(y / len); lp.light[l].vec[2] = (float)(z / len);
+        }
+    }
+    FrameParams fr;
+    fr.pos_fp = reinterpret_cast<const float4*>(g->pos_fp);
+    fr.nrm_u = reinterpret_cast<const float4*>(g->nrm_u);
+    fr.tan_v = reinterpret_cast<const float4*>(g->tan_v);
+    fr.material = g->material;
+    fr.n_pixels = npx;
+    fr.cam[0] = g->cam_pos[0]; fr.cam[1] = g->cam_pos[1]; fr.cam[2] = g->cam_pos[2];
+    const NetParams net = net_params(ctx);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_shade_fp32(net, fr, lp, radiance_dev, s);
+    else e = launch_shade_tc(net, ctx->cfg.precision, ctx->num_sms, fr, lp, radiance_dev, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_shade_frame launch", e);
+    ctx->launches += 1;
+    return NBSDF_OK;
+}

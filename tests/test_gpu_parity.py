@@ -1,0 +1,256 @@
+"""Parity of the CUDA path (through the C ABI, via the ctypes binding) against the fp64 oracle.  -m gpu.
+
+Tolerances are BASELINE.json north_star's: per channel, rel = |gpu - ref| / max(|ref|, 1e-6);
+tensor-core precisions (bf16 / fp16): max <= 1e-2 and mean <= 2e-3;  fp32 CUDA-core variant: max <= 1e-5.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_2406_17782_b200 import api, synth  # noqa: E402
+
+TOL = {"fp32": (1e-5, 1e-5), "bf16": (1e-2, 2e-3), "fp16": (1e-2, 2e-3)}
+PRECS = ["fp32", "fp16", "bf16"]
+
+
+def rel_err(gpu, ref):
+    gpu = np.asarray(gpu, np.float64).reshape(-1, 3)
+    ref = np.asarray(ref, np.float64).reshape(-1, 3)
+    r = np.abs(gpu - ref) / np.maximum(np.abs(ref), 1e-6)
+    return r.max(axis=0), r.mean(axis=0)
+
+
+def check(gpu, ref, prec, what=""):
+    assert np.isfinite(gpu).all(), what
+    mx, mean = rel_err(gpu, ref)
+    tmax, tmean = TOL[prec]
+    assert (mx <= tmax).all() and (mean <= tmean).all(), f"{what} {prec}: max {mx} mean {mean}"
+    return mx, mean
+
+
+class Ctx:
+    def __init__(self, cfg, prec, L=16, H=64, M=None):
+        M = cfg["latents"].shape[0] if M is None else M
+        self.ctx = api.nbsdf_create(cfg["weights"], cfg["biases"], L, H, M, prec)
+        api.nbsdf_set_latents(self.ctx, 0, cfg["latents"])
+
+    def eval(self, q, frames=None):
+        n = len(q)
+        qd = api.queries_to_device(q) if n else None
+        fd = torch.from_numpy(np.ascontiguousarray(frames, np.float32)).cuda() if frames is not None and n else None
+        out = torch.full((max(n, 1), 3), float("nan"), dtype=torch.float32, device="cuda")
+        api.nbsdf_eval(self.ctx, qd, fd, n, out if n else None)
+        torch.cuda.synchronize()
+        return out[:n].cpu().numpy()
+
+    def shade(self, g, lights):
+        gd = api.gbuffer_to_device(g)
+        npx = g["width"] * g["height"]
+        out = torch.full((npx, 3), float("nan"), dtype=torch.float32, device="cuda")
+        api.nbsdf_shade_frame(self.ctx, gd, lights, out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+    def close(self):
+        api.nbsdf_destroy(self.ctx)
+
+
+@pytest.fixture(scope="module")
+def cfg0():
+    return synth.config(0)
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_config0_tiny_eval(cfg0, prec):
+    ref = oracle.eval_queries(cfg0["weights"], cfg0["biases"], cfg0["latents"], cfg0["queries"])
+    c = Ctx(cfg0, prec)
+    out = c.eval(cfg0["queries"])
+    c.close()
+    check(out, ref, prec, "config 0")
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_tile_edges_and_empty(cfg0, prec):
+    c = Ctx(cfg0, prec)
+    for n in (0, 1, 127, 128, 129, 4097 - 1024, 513):
+        q = synth.make_queries(np.random.default_rng(n), n, 1)
+        out = c.eval(q)
+        assert out.shape == (n, 3)
+        if n:
+            ref = oracle.eval_queries(cfg0["weights"], cfg0["biases"], cfg0["latents"], q)
+            check(out, ref, prec, f"n={n}")
+    c.close()
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_frames_materials_background_and_wrap(prec):
+    cfg = synth.config(1, n=3000)
+    rng = np.random.default_rng(77)
+    q = cfg["queries"].copy()
+    q["u"] = rng.uniform(-4, 4, len(q)); q["v"] = rng.uniform(-4, 4, len(q))      # exercised wrap
+    q["footprint"][:8] = [0.0, -1.0, 1e-30, 100.0, 16.0, 2.0 ** -20, 1.0, 3.0]     # clamp edges
+    q["material"][5::17] = -1
+    fr = synth.make_frames(rng, len(q))
+    fr[1, 3:] = fr[1, :3] * 2.0                                                     # degenerate tangent hint
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], q, fr)
+    c = Ctx(cfg, prec)
+    out = c.eval(q, fr)
+    assert (out[5::17] == 0).all()
+    live = q["material"] >= 0
+    check(out[live], ref[live], prec, "frames")
+    # no frames == identity frames
+    ident = np.tile(np.array([0, 0, 1, 1, 0, 0], np.float32), (len(q), 1))
+    a, b = c.eval(q), c.eval(q, ident)
+    np.testing.assert_allclose(a, b, rtol=1e-6 if prec == "fp32" else 1e-2)
+    c.close()
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_batch_permutation_gives_identical_bits(prec):
+    cfg = synth.config(1, n=5000)
+    c = Ctx(cfg, prec)
+    q = cfg["queries"]
+    perm = np.random.default_rng(5).permutation(len(q))
+    a = c.eval(q)
+    b = c.eval(q[perm])
+    c.close()
+    np.testing.assert_array_equal(a[perm].view(np.uint32), b.view(np.uint32))
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_config2_small_frame(prec):
+    cfg = synth.config(2, width=320, height=136)
+    g = cfg["gbuffer"]
+    g["material"] = g["material"].copy(); g["material"][7::53] = -1
+    ref = oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, cfg["lights"])
+    c = Ctx(cfg, prec)
+    out = c.shade(g, cfg["lights"])
+    assert (out[7::53] == 0).all()
+    live = g["material"] >= 0
+    check(out[live], ref[live], prec, "frame")
+    # zero lights -> black frame
+    assert (c.shade(g, cfg["lights"][:0]) == 0).all()
+    c.close()
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_mlp_a_reuse_matches_eval_on_expanded_queries(prec):
+    """The frame kernel evaluates MLP-A once per pixel; nbsdf_eval on the expanded (pixel, light) list does not."""
+    cfg = synth.config(2, width=64, height=40)
+    g, lights = cfg["gbuffer"], cfg["lights"][:1]            # one directional light: E = 1, wi constant
+    c = Ctx(cfg, prec)
+    frame = c.shade(g, lights)
+    npx = 64 * 40
+    x = g["pos_fp"][:, :3].astype(np.float64)
+    wo = g["cam_pos"].astype(np.float64)[None] - x
+    wo /= np.linalg.norm(wo, axis=1, keepdims=True)
+    q = np.zeros(npx, dtype=synth.QUERY_DTYPE)
+    q["u"], q["v"], q["footprint"], q["material"] = g["nrm_u"][:, 3], g["tan_v"][:, 3], g["pos_fp"][:, 3], g["material"]
+    q["wi"] = np.tile(lights[0]["vec"], (npx, 1)); q["wo"] = wo
+    frames = np.concatenate([g["nrm_u"][:, :3], g["tan_v"][:, :3]], 1)
+    rgb = c.eval(q, frames)
+    c.close()
+    n = g["nrm_u"][:, :3].astype(np.float64)
+    cos = np.maximum((q["wi"].astype(np.float64) * n).sum(1) / np.linalg.norm(n, axis=1), 0)[:, None]
+    np.testing.assert_allclose(frame, rgb * cos, rtol=2e-5 if prec == "fp32" else 2e-2, atol=1e-6)
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_config3_editing_small(prec):
+    cfg = synth.config(3, width=256, height=192)
+    g, lights = cfg["gbuffer"], cfg["lights"]
+    c = Ctx(cfg, prec)
+    f1 = c.shade(g, lights)
+    ref1 = oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, lights)
+    check(f1, ref1, prec, "frame 1")
+    m = cfg["edit_material"]
+    api.nbsdf_set_latents(c.ctx, m, cfg["edit_latent"])
+    f2 = c.shade(g, lights)
+    c.close()
+    Z2 = cfg["latents"].copy(); Z2[m] = cfg["edit_latent"]
+    ref2 = oracle.shade_frame(cfg["weights"], cfg["biases"], Z2, g, lights)
+    check(f2, ref2, prec, "frame 2")
+    same = g["material"] != m
+    np.testing.assert_array_equal(f1[same].view(np.uint32), f2[same].view(np.uint32))   # untouched materials: same bits
+    assert (f1[~same] != f2[~same]).any()
+
+
+@pytest.mark.parametrize("H", [32, 64, 128])
+@pytest.mark.parametrize("L", [8, 16, 32])
+@pytest.mark.parametrize("prec", PRECS)
+def test_config4_dims(prec, L, H):
+    seed = synth.sweep_seed(0, [32, 64, 128].index(H), [8, 16, 32].index(L))
+    cfg = synth.config(4, n=1500, L=L, H=H, seed=seed)
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"])
+    c = Ctx(cfg, prec, L=L, H=H)
+    out = c.eval(cfg["queries"])
+    g = synth.make_gbuffer(np.random.default_rng(seed), 96, 40)
+    lights = synth.lights_direct5()
+    fr = c.shade(g, lights)
+    c.close()
+    check(out, ref, prec, f"L={L} H={H}")
+    check(fr, oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, lights), prec, f"frame L={L} H={H}")
+
+
+@pytest.mark.parametrize("prec", ["fp16", "bf16"])
+def test_config1_full_size(prec):
+    """2^20 queries in the launch configuration bench.py times; every output checked against the oracle."""
+    cfg = synth.config(1)
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"])
+    c = Ctx(cfg, prec)
+    out = c.eval(cfg["queries"])
+    c.close()
+    mx, mean = check(out, ref, prec, "config 1")
+    print(f"config 1 {prec}: max rel {mx}, mean rel {mean}")
+
+
+@pytest.mark.parametrize("prec", ["fp16"])
+def test_config2_and_3_full_size_sampled(prec):
+    """Full-size frames in bench.py's launch configuration; oracle on a seeded sample of whole rows."""
+    for idx, n_rows in ((2, 48), (3, 24)):
+        cfg = synth.config(idx)
+        g, lights = cfg["gbuffer"], cfg["lights"]
+        c = Ctx(cfg, prec)
+        out = c.shade(g, lights)
+        c.close()
+        assert np.isfinite(out).all() and (out > 0).all()
+        W, Hh = g["width"], g["height"]
+        rows = np.random.default_rng(idx).choice(Hh, n_rows, replace=False)
+        rows = np.concatenate([rows, [0, 63, 64, Hh - 1]])           # include tile edges and the last row
+        for r in rows:
+            ref = oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, lights, first=int(r) * W, count=W)
+            check(out[int(r) * W:(int(r) + 1) * W], ref, prec, f"config {idx} row {r}")
+
+
+def test_error_codes_and_no_fallback(cfg0):
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_create(cfg0["weights"], cfg0["biases"], 16, 64, 0)
+    assert e.value.status == api.NBSDF_E_UNSUPPORTED
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_create(cfg0["weights"], cfg0["biases"], 16, 64, 1, device=99)
+    assert e.value.status == api.NBSDF_E_INVALID
+    c = Ctx(cfg0, "fp16")
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_set_latents(c.ctx, 1, cfg0["latents"])               # first + count > max_materials
+    assert e.value.status == api.NBSDF_E_INVALID
+    out = torch.empty((4, 3), device="cuda")
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_eval(c.ctx, None, None, 4, out)
+    assert e.value.status == api.NBSDF_E_INVALID
+    qd = api.queries_to_device(cfg0["queries"][:8])
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_eval(c.ctx, qd[4:], None, 4, out)                      # misaligned
+    assert e.value.status == api.NBSDF_E_INVALID
+    g = api.gbuffer_to_device(synth.make_gbuffer(np.random.default_rng(0), 8, 8))
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_shade_frame(c.ctx, g, np.zeros(33, synth.LIGHT_DTYPE), torch.empty((64, 3), device="cuda"))
+    assert e.value.status == api.NBSDF_E_INVALID
+    n0 = api.nbsdf_launch_count(c.ctx)
+    api.nbsdf_eval(c.ctx, qd, None, 8, torch.empty((8, 3), device="cuda"))
+    assert api.nbsdf_launch_count(c.ctx) == n0 + 1
+    torch.cuda.synchronize()
+    c.close()

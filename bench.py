@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the nbsdf hot path on B200.
+
+A step is one pass of the fused decoder (stages A1-A4, B1-B7: `nbsdf_eval`) over one batch of BASELINE.json
+configs[1]: 2^20 synthetic queries, 8 materials, L=16, H=64, weights stored in bf16, fp32 I/O.  `value` is whole-job
+decoder BSDF queries/s with inputs resident in HBM; `e2e` is the same metric through the same C-ABI call with HOST
+buffers (pinned host -> device copy of the batch and device -> host read of the result inside the timed region).
+The same JSON line also carries the other half of BASELINE.json's metric, the 1920x1080 five-light frame time
+(`nbsdf_shade_frame`, stages C1-C3 on configs[2]), timed the same way in its own loop.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--precision fp16|bf16|fp32] [--impl ours|reference]
+
+Under torchrun (N > 1) every rank processes its own batch (weak scaling, no data-path collective) and the time is
+the max over ranks.  `--impl reference` times the fp64 oracle (oracle/, as it stands) on the host cores.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_QUERY = 2 * (19 * 64 + 64 * 64 + 64 * 32 + 38 * 64 + 64 * 64 + 64 * 3)        # 28 160, unpadded
+FLOP_MLP_A = 2 * (19 * 64 + 64 * 64 + 64 * 32)                                          # 14 720
+FLOP_MLP_B = 2 * (38 * 64 + 64 * 64 + 64 * 3)                                           # 13 440
+BYTES_PER_QUERY = 40 + 12
+N_ROTATE = 8            # distinct resident batches cycled through so that no step finds its input in L2
+METRIC = "decoder_bsdf_queries_per_sec"
+UNIT = "queries/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"bf16_tflops": float(d["bf16_tflops"]), "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", 0)),
+                "hbm_gbs": float(d["hbm_gbs"]), "source": "measured"}
+    return {"bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "hbm_gbs": 6650.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML every few ms while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz, self._stop, self._t = [], set(), None, threading.Event(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _reasons(self):
+        nv = self.nv
+        try:
+            mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+        except Exception:
+            try:
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            except Exception:
+                return []
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting"}
+        return [v for k, v in names.items() if mask & k]
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                self.reasons.update(self._reasons())
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def start(self):
+        if self.nv is not None:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t is not None:
+            self._t.join()
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_rate(cfg, n_sample, threads=0):
+    """queries/s of the fp64 oracle, as it stands, on the first n_sample queries of cfg."""
+    import oracle
+    q = cfg["queries"][:n_sample]
+    t0 = time.perf_counter()
+    oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], q, n_threads=threads)
+    dt = time.perf_counter() - t0
+    return len(q) / dt, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step a bounded sample of configs[1]."""
+    from paper_2406_17782_b200 import dist, synth
+    rank, _, world = dist.env_world()
+    if rank != 0:
+        return
+    import oracle
+    cores = len(os.sched_getaffinity(0))
+    cfg = synth.config(1, n=1 << 18)
+    rate0, _ = oracle_rate(cfg, 1 << 13)
+    budget_s = 150.0
+    n_step = int(min(1 << 18, max(256, rate0 * budget_s / max(1, args.steps + args.warmup))))
+    for _ in range(args.warmup):
+        oracle_rate(cfg, n_step)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"][:n_step])
+    dt = time.perf_counter() - t0
+    value = n_step * args.steps / dt
+    sample = f"first {n_step} of the 2^20 queries of configs[1] per step, fp64, OpenMP over queries"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1] batch eval (bounded sample per step)", "queries_per_step": n_step,
+                       "latent_dim": 16, "hidden": 64, "materials": 8},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def time_loop(torch, fn, steps, barrier):
+    """barrier + sync, K calls of fn(i) timed with CUDA events on the current stream, sync + barrier.  Returns ms."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(steps):
+        fn(i)
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def run_ours(args):
+    import torch
+    from paper_2406_17782_b200 import api, dist, synth
+
+    rank, local_rank, world = dist.init("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    peaks = measured_peaks()
+    prec = args.precision
+    K, W = args.steps, max(args.warmup, 3)
+
+    # ---- workload: configs[1], one distinct batch set per rank (weak scaling) ----
+    n = 1 << 20
+    cfg = synth.config(1, n=n, seed=dist.rank_seed(1, rank))
+    ctx = api.nbsdf_create(cfg["weights"], cfg["biases"], 16, 64, 8, prec, device=local_rank)
+    api.nbsdf_set_latents(ctx, 0, cfg["latents"])
+    q_host = torch.from_numpy(cfg["queries"].view(np.uint8).reshape(-1).copy()).pin_memory()
+    # N_ROTATE distinct device batches (rotations of the same records: same distribution, different addresses/order)
+    q_dev = []
+    for r in range(N_ROTATE):
+        qr = np.roll(cfg["queries"], r * 12345)
+        q_dev.append(torch.from_numpy(qr.view(np.uint8).reshape(-1).copy()).to(dev))
+    out_dev = [torch.empty((n, 3), dtype=torch.float32, device=dev) for _ in range(N_ROTATE)]
+    barrier = dist.barrier
+
+    def step(i):
+        api.nbsdf_eval(ctx, q_dev[i % N_ROTATE], None, n, out_dev[i % N_ROTATE])
+
+    for i in range(W):
+        step(i)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    l0 = api.nbsdf_launch_count(ctx)
+    sampler.start()
+    ms = time_loop(torch, step, K, barrier)
+    clocks = sampler.stop()
+    launches = api.nbsdf_launch_count(ctx) - l0
+    ms = dist.max_over_ranks(ms, dev)
+    value = world * n * K / (ms * 1e-3)
+
+    # ---- e2e: HOST buffers through the same call; H2D of the batch and D2H of the result inside the timed region ----
+    out_host = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    q_stage = torch.empty_like(q_dev[0])
+    o_stage = out_dev[0]
+
+    def step_e2e(i):
+        q_stage.copy_(q_host, non_blocking=True)
+        api.nbsdf_eval(ctx, q_stage, None, n, o_stage)
+        out_host.copy_(o_stage, non_blocking=True)
+
+    k_e2e = max(3, min(K, 50))
+    for i in range(3):
+        step_e2e(i)
+    torch.cuda.synchronize()
+    ms_e2e = dist.max_over_ranks(time_loop(torch, step_e2e, k_e2e, barrier), dev)
+    e2e_value = world * n * k_e2e / (ms_e2e * 1e-3)
+
+    # ---- the other half of the metric: 1080p, 5 lights (configs[2]) ----
+    fcfg = synth.config(2, seed=dist.rank_seed(2, rank))
+    fctx = api.nbsdf_create(fcfg["weights"], fcfg["biases"], 16, 64, 8, prec, device=local_rank)
+    api.nbsdf_set_latents(fctx, 0, fcfg["latents"])
+    g = fcfg["gbuffer"]
+    npx = g["width"] * g["height"]
+    gds, rads = [], []
+    for r in range(3):                               # 3 x (108 + 25) MB > L2
+        gr = {k: np.roll(g[k], r * 4099, axis=0) for k in ("pos_fp", "nrm_u", "tan_v", "material")}
+        gr.update(width=g["width"], height=g["height"], cam_pos=g["cam_pos"])
+        gds.append(api.gbuffer_to_device(gr, dev))
+        rads.append(torch.empty((npx, 3), dtype=torch.float32, device=dev))
+
+    def fstep(i):
+        api.nbsdf_shade_frame(fctx, gds[i % 3], fcfg["lights"], rads[i % 3])
+
+    kf = max(3, min(K, 200))
+    for i in range(3):
+        fstep(i)
+    torch.cuda.synchronize()
+    fms = dist.max_over_ranks(time_loop(torch, fstep, kf, barrier), dev) / kf
+
+    line = None
+    if rank == 0:
+        us_per_launch = 1e3 * ms / K
+        achieved_tf = FLOP_PER_QUERY * n / (us_per_launch * 1e-6) / 1e12
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get(f"eval_{prec}_dram_bytes_per_launch")
+        frame_flop = npx * (FLOP_MLP_A + 5 * FLOP_MLP_B)
+        frame_tf = frame_flop / (fms * 1e-3) / 1e12
+        cores = len(os.sched_getaffinity(0))
+        n_cpu = 1 << 18
+        cpu_rate, cpu_dt = oracle_rate(cfg, n_cpu)
+        import oracle
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": {"fp16": "f16", "bf16": "bf16", "fp32": "f32"}[prec], "data": "synthetic",
+            "config": {"workload": "configs[1]: batch eval, 2^20 queries/step/GPU, 8 materials, L=16, H=64, F=32, "
+                                   "bf16-stored weights, fp32 I/O", "queries_per_step_per_gpu": n, "precision": prec,
+                       "l2": f"inputs rotate over {N_ROTATE} distinct resident batches "
+                             f"({N_ROTATE * n * BYTES_PER_QUERY / 1e6:.0f} MB > 126 MB L2), no flush kernel",
+                       "parallelism": f"replicated weights, {world} independent query shards"},
+            "roofline": {"bound": "tensor" if prec != "fp32" else "alu", "achieved": achieved_tf,
+                         "peak": peaks["bf16_tflops"] if prec != "fp32" else 74.4, "unit": "TFLOP/s",
+                         "frac": achieved_tf / (peaks["bf16_tflops"] if prec != "fp32" else 74.4),
+                         "traffic": traffic, "peak_source": peaks["source"] + " burst (cuBLAS bf16 8192^3)",
+                         "frac_of_sustained": achieved_tf / peaks["bf16_tflops_sustained"] if peaks["bf16_tflops_sustained"] else None,
+                         "kernel": "tc_kernel<16,64,...,eval>" if prec != "fp32" else "eval_fp32_kernel",
+                         "us_per_launch": us_per_launch, "flop_per_query": FLOP_PER_QUERY,
+                         "hbm_gbs_algorithmic": BYTES_PER_QUERY * n / (us_per_launch * 1e-6) / 1e9},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(q_host.numel()),
+                    "d2h_bytes_per_step": int(out_host.numel() * 4), "steps": k_e2e},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "frame": {"workload": "configs[2]: 1920x1080, 8 materials in 64px tiles, 1 directional + 4 point lights",
+                      "frame_ms": fms, "steps": kf, "flop_per_pixel": FLOP_MLP_A + 5 * FLOP_MLP_B,
+                      "achieved_tflops": frame_tf, "frac": frame_tf / peaks["bf16_tflops"] if prec != "fp32" else frame_tf / 74.4,
+                      "decoder_evals_per_s": world * npx * 5 / (fms * 1e-3)},
+            "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle",
+                             "sample": f"first {n_cpu} of the 2^20 queries of configs[1], fp64, OpenMP over queries, {cpu_dt:.1f} s"},
+        }
+    api.nbsdf_destroy(ctx)
+    api.nbsdf_destroy(fctx)
+    dist.finalize()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--precision", default="fp16", choices=["fp16", "bf16", "fp32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

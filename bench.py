@@ -241,7 +241,7 @@ def run_ours(args):
         frame_flop = npx * (FLOP_MLP_A + 5 * FLOP_MLP_B)
         frame_tf = frame_flop / (fms * 1e-3) / 1e12
         cores = len(os.sched_getaffinity(0))
-        n_cpu = 1 << 18
+        n_cpu = 1 << 20
         cpu_rate, cpu_dt = oracle_rate(cfg, n_cpu)
         import oracle
         line = {

@@ -134,33 +134,46 @@ cudaError_t launch_shade_tc(const NetParams& net, int precision, int num_sms, co
 cudaError_t init_tc(int L, int H);       // cudaFuncSetAttribute for the instantiations in use
 cudaError_t init_fp32();
 
-// shared-memory image layout of the tensor path, computed identically on host (packing) and device (carving)
+// shared-memory image layout of the tensor path, computed identically on host (packing) and device (carving).
+// Biases are folded into the contractions: every layer's input vector is extended by kBiasCols constant entries
+// (c0, c1, c2) and the weight rows by (b0/c0, b1/c1, b2/c2), where b0 + b1 + b2 is the 16-bit three-way split of
+// the fp32 bias -- the tensor core then adds the bias in its fp32 accumulator at full precision and the epilogue
+// is left with ReLU + pack only.  Layers 1 and 4 take the constants inside their K padding; the K = H layers get
+// one extra 16-wide K step whose A operand is a per-warpgroup constant TMEM block.
+constexpr int kBiasCols = 3;
+
+// constant fed in bias input column j: fp16 scales the residual parts up out of the subnormal range
+__host__ __device__ constexpr float tc_bias_const(bool bf16, int j)
+{
+    return bf16 ? 1.0f : (j == 0 ? 1.0f : (j == 1 ? 0.000244140625f /* 2^-12 */ : 0.00006103515625f /* 2^-14 */));
+}
+
 struct TcLayout {
-    int K1p, K4p;            // padded K of layers 1 and 4 (multiples of 16)
+    int K1p, K4p;            // padded K of layers 1 and 4 (multiples of 16), bias columns included
+    int Kp[6];               // padded K of every layer as issued (K = H layers: H + 16)
+    int Kbias[6];            // input index of the first bias column of every layer
     uint32_t w_off[6];       // byte offset of each layer's weight tiles (1024-aligned)
     uint32_t w_rows[6];      // padded N (rows) of each layer
-    uint32_t bias_off[6];    // byte offset of each layer's fp32 biases
     uint32_t total;          // bytes of the image (multiple of 16)
 };
 
-__host__ __device__ inline int pad16(int k) { return (k + 15) & ~15; }
+__host__ __device__ constexpr int pad16(int k) { return (k + 15) & ~15; }
 
-__host__ __device__ inline TcLayout tc_layout(int L, int H)
+__host__ __device__ constexpr TcLayout tc_layout(int L, int H)
 {
-    TcLayout t;
-    t.K1p = pad16(L + 3);
-    t.K4p = pad16(kFeat + 6);
-    const int K[6] = { t.K1p, H, H, t.K4p, H, H };
+    TcLayout t{};
+    t.K1p = pad16(L + 3 + kBiasCols);
+    t.K4p = pad16(kFeat + 6 + kBiasCols);
+    const int K[6] = { t.K1p, H + 16, H + 16, t.K4p, H + 16, H + 16 };
+    const int Kb[6] = { L + 3, H, H, kFeat + 6, H, H };
     const int N[6] = { H, H, kFeat, H, H, 16 };
     uint32_t off = 0;
     for (int l = 0; l < 6; ++l) {
+        t.Kp[l] = K[l];
+        t.Kbias[l] = Kb[l];
         t.w_off[l] = off;
         t.w_rows[l] = (uint32_t)N[l];
         off += (uint32_t)((K[l] + 63) / 64) * (uint32_t)N[l] * 128u;   // N rows x 128 B per 64-wide K block
-    }
-    for (int l = 0; l < 6; ++l) {
-        t.bias_off[l] = off;
-        off += (uint32_t)N[l] * 4u;
     }
     t.total = (off + 15u) & ~15u;
     return t;

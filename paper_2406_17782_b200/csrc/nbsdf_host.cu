@@ -52,28 +52,40 @@ static uint16_t to_op16(float v, bool bf16)
     return __half_as_ushort(__float2half_rn(v));
 }
 
+static float from_op16(uint16_t bits, bool bf16)
+{
+    if (bf16) return __bfloat162float(__ushort_as_bfloat16(bits));
+    return __half2float(__ushort_as_half(bits));
+}
+
 // Shared-memory image of the tensor path: per layer, per 64-wide K block, N rows of 128 bytes, K-major, with the
-// 16-byte chunk index XOR-ed by (row % 8) (the 128-byte swizzle tcgen05 applies when it reads the tile), then biases.
+// 16-byte chunk index XOR-ed by (row % 8) (the 128-byte swizzle tcgen05 applies when it reads the tile).
+// Columns [Kbias, Kbias + 3) of every row hold the three-way 16-bit split of the fp32 bias, each part divided by
+// the constant the kernel feeds in that input column (tc_bias_const), so that sum_j w_j * c_j == bias to ~2^-24.
 static void pack_tc(int L, int H, bool bf16, const nbsdf_weights* w, uint8_t* img)
 {
     const TcLayout lay = tc_layout(L, H);
     const int Kr[6] = { L + 3, H, H, kFeat + 6, H, H };
-    const int Kp[6] = { lay.K1p, H, H, lay.K4p, H, H };
     const int Nr[6] = { H, H, kFeat, H, H, 3 };
     memset(img, 0, lay.total);
-    for (int l = 0; l < 6; ++l) {
+    auto put = [&](int l, int n, int k, uint16_t bits) {
         const int Np = (int)lay.w_rows[l];
+        const int kb = k / 64, kk = k % 64;
+        const int chunk = (kk / 8) ^ (n % 8);
+        const size_t off = lay.w_off[l] + (size_t)kb * Np * 128 + (size_t)n * 128 + (size_t)chunk * 16 + (size_t)(kk % 8) * 2;
+        memcpy(img + off, &bits, 2);
+    };
+    for (int l = 0; l < 6; ++l) {
         for (int n = 0; n < Nr[l]; ++n) {
-            for (int k = 0; k < Kr[l]; ++k) {
-                const int kb = k / 64, kk = k % 64;
-                const int chunk = (kk / 8) ^ (n % 8);
-                const size_t off = lay.w_off[l] + (size_t)kb * Np * 128 + (size_t)n * 128 + (size_t)chunk * 16 + (size_t)(kk % 8) * 2;
-                const uint16_t bits = to_op16(w->W[l][(size_t)n * Kr[l] + k], bf16);
-                memcpy(img + off, &bits, 2);
+            for (int k = 0; k < Kr[l]; ++k) put(l, n, k, to_op16(w->W[l][(size_t)n * Kr[l] + k], bf16));
+            double r = (double)w->b[l][n];
+            for (int j = 0; j < kBiasCols; ++j) {
+                const double c = (double)tc_bias_const(bf16, j);
+                const uint16_t bits = to_op16((float)(r / c), bf16);
+                put(l, n, lay.Kbias[l] + j, bits);
+                r -= (double)from_op16(bits, bf16) * c;
             }
-            memcpy(img + lay.bias_off[l] + (size_t)n * 4, &w->b[l][n], 4);
         }
-        (void)Kp;
     }
 }
 

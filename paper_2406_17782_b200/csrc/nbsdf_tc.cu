@@ -6,7 +6,7 @@
 //   A (activations) in TENSOR MEMORY, written by the owning thread with tcgen05.st as packed 16-bit pairs,
 //   B (weights)     resident in shared memory for the whole kernel as 128-byte-swizzled K-major UMMA tiles,
 //   D (accumulator) fp32 in tensor memory, read back with tcgen05.ld by the owning thread,
-// so the inter-layer epilogue (bias, ReLU, 16-bit pack) is thread-local and no activation ever touches shared
+// so the inter-layer epilogue (ReLU, 16-bit pack) is thread-local and no activation ever touches shared
 // memory or HBM.  Query tiles stream in with cp.async.bulk (TMA bulk copy) one tile ahead.  Warpgroups are not
 // specialised: each alternates "issue MMAs / wait / epilogue", and the NWG warpgroups of a CTA interleave so that
 // the tensor pipe, the TMEM load path and the FP32 pipes overlap across tiles.
@@ -14,7 +14,9 @@
 // TMEM columns per warpgroup (512 / NWG available):
 //   [0, H)                 accumulator (N <= H fp32 columns)
 //   [H, H + H/2)           AH: hidden activations as A operand (K = H 16-bit values = H/2 columns)
-//   [H + H/2, +24)         AY: layer-1 input x = [z, u', v', lf] (K1p/2 columns) and later y = [feat, wi, wo] (24 columns)
+//   [H + H/2, +8)          constant block (c0, c1, c2, 0, ...): A operand of the bias K step of the K = H layers
+//   [H + H/2 + 8, +24)     AY: layer-1 input x = [z, u', v', lf, c] (K1p/2 columns), later y = [feat, wi, wo, c] (24 columns)
+// Biases ride inside the contractions (see tc_layout in nbsdf_common.cuh): the epilogue is ReLU + 16-bit pack only.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
@@ -178,34 +180,23 @@ __host__ __device__ constexpr uint32_t make_idesc(int N)
 // ------------------------------------------------------------------------------------------------
 template <int L, int H, bool kBf16, int NWG>
 struct Tc {
-    static constexpr int K1p = (L + 3 + 15) & ~15;
-    static constexpr int K4p = 48;
+    static constexpr TcLayout kLay = tc_layout(L, H);
+    static constexpr int K1p = kLay.K1p;
+    static constexpr int K4p = kLay.K4p;
     static constexpr int kThreads = NWG * 128;
     static constexpr int kColsPerWg = 512 / NWG;
     static constexpr int kAccCol = 0;
-    static constexpr int kAhCol = H;
-    static constexpr int kAyCol = H + H / 2;
+    static constexpr int kAhCol = H;                 // hidden activations, H/2 columns
+    static constexpr int kOneCol = H + H / 2;        // constant block (c0, c1, c2, 0...): the bias K step of the K = H layers
+    static constexpr int kAyCol = kOneCol + 8;       // x = [z, u', v', lf, c] and later y = [feat, wi, wo, c]
     static_assert(kAyCol + 24 <= kColsPerWg, "TMEM budget per warpgroup");
     static_assert(L % 8 == 0 && H % 32 == 0, "dims");
+    static_assert(K1p <= 48 && K4p == 48, "AY holds at most 24 columns");
 
     static constexpr uint32_t kLatBytes = 64 * 32 * 2;            // packed latent table, max M x max L
     static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);
 
-    struct Smem {
-        uint32_t wimg, lat, stage, bars, tmem_ptr;                // shared-space byte addresses
-        const uint8_t* g_wimg; const uint8_t* g_lat; const uint8_t* g_stage;   // generic pointers
-    };
-
-    __host__ __device__ static constexpr uint32_t wimg_bytes()
-    {
-        // mirrors tc_layout(L, H).total
-        uint32_t off = 0;
-        const int K[6] = { K1p, H, H, K4p, H, H };
-        const int N[6] = { H, H, kFeat, H, H, 16 };
-        for (int l = 0; l < 6; ++l) off += (uint32_t)((K[l] + 63) / 64) * (uint32_t)N[l] * 128u;
-        for (int l = 0; l < 6; ++l) off += (uint32_t)N[l] * 4u;
-        return (off + 15u) & ~15u;
-    }
+    __host__ __device__ static constexpr uint32_t wimg_bytes() { return kLay.total; }
     __host__ __device__ static constexpr uint32_t smem_bytes()
     {
         return 1024u + ((wimg_bytes() + 127u) & ~127u) + kLatBytes + NWG * kStageBytes + 256u;
@@ -213,22 +204,26 @@ struct Tc {
 };
 
 // Issues the MMAs of one layer for this warpgroup's tile and commits them to the warpgroup's mbarrier.
-// Called by ONE thread.  a_tmem / d_tmem are lane-0 TMEM addresses; w_saddr the layer's tiles in shared memory.
-template <bool kBf16>
-__device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t a_tmem, uint32_t w_saddr, int K, int N, uint32_t bar)
+// Called by ONE thread.  K/16 steps in total; the first KA/16 read the A operand at a_tmem, the remaining ones
+// (the bias step of the K = H layers) read the constant block at one_tmem.  d_tmem/a_tmem/one_tmem are lane-0
+// TMEM addresses; w_saddr is the layer's weight tiles in shared memory.
+template <bool kBf16, int K, int N, int KA>
+__device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t a_tmem, uint32_t one_tmem, uint32_t w_saddr, uint32_t bar)
 {
-    const uint32_t idesc = make_idesc<kBf16>(N);
+    constexpr uint32_t idesc = make_idesc<kBf16>(N);
     tc_fence_after();
+#pragma unroll
     for (int s = 0; s < K / 16; ++s) {
         const uint32_t b = w_saddr + (uint32_t)(s >> 2) * (uint32_t)N * 128u + (uint32_t)(s & 3) * 32u;
-        umma_ts(d_tmem, a_tmem + (uint32_t)s * 8u, make_b_desc(b), idesc, s > 0 ? 1u : 0u);
+        const uint32_t a = s < KA / 16 ? a_tmem + (uint32_t)s * 8u : one_tmem + (uint32_t)(s - KA / 16) * 8u;
+        umma_ts(d_tmem, a, make_b_desc(b), idesc, s > 0 ? 1u : 0u);
     }
     umma_commit(bar);
 }
 
-// Epilogue of a hidden layer: acc (N fp32 columns) + bias -> (ReLU) -> packed 16-bit pairs -> A operand columns.
+// Epilogue of a hidden layer: acc (N fp32 columns, bias already inside) -> (ReLU) -> packed 16-bit pairs -> A columns.
 template <int N, bool kRelu, bool kBf16>
-__device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_taddr, const float* bias)
+__device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_taddr)
 {
 #pragma unroll
     for (int c = 0; c < N; c += 32) {
@@ -237,11 +232,8 @@ __device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_tad
         tmem_wait_ld();
         uint32_t p[16];
 #pragma unroll
-        for (int j = 0; j < 16; j += 2) {
-            const float4 b4 = *reinterpret_cast<const float4*>(bias + c + 2 * j);
-            p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]) + b4.x, __uint_as_float(v[2 * j + 1]) + b4.y);
-            p[j + 1] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j + 2]) + b4.z, __uint_as_float(v[2 * j + 3]) + b4.w);
-        }
+        for (int j = 0; j < 16; ++j)
+            p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
         tmem_st16(a_taddr + c / 2, p);
     }
 }
@@ -310,11 +302,15 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const uint32_t col0 = tmem_base + (uint32_t)(wg * T::kColsPerWg);                 // lane 0: for MMA operands
     const uint32_t lane_taddr = col0 + ((uint32_t)((warp & 3) * 32) << 16);           // this warp's lane quarter
     const uint32_t acc_t = lane_taddr + T::kAccCol, ah_t = lane_taddr + T::kAhCol, ay_t = lane_taddr + T::kAyCol;
-    const uint32_t acc_d = col0 + T::kAccCol, ah_d = col0 + T::kAhCol, ay_d = col0 + T::kAyCol;
+    const uint32_t acc_d = col0 + T::kAccCol, ah_d = col0 + T::kAhCol, ay_d = col0 + T::kAyCol, one_d = col0 + T::kOneCol;
 
-    const float* bias[6];
-#pragma unroll
-    for (int l = 0; l < 6; ++l) bias[l] = reinterpret_cast<const float*>(g_wimg + lay.bias_off[l]);
+    // bias constants (c0, c1, c2) as packed pairs; the constant block is written once per kernel
+    const uint32_t c01 = pack2<kBf16, false>(tc_bias_const(kBf16, 0), tc_bias_const(kBf16, 1));
+    const uint32_t c2z = pack2<kBf16, false>(tc_bias_const(kBf16, 2), 0.0f);
+    {
+        uint32_t ones[8] = { c01, c2z, 0u, 0u, 0u, 0u, 0u, 0u };
+        tmem_st8(lane_taddr + T::kOneCol, ones);
+    }
     uint32_t w_s[6];
 #pragma unroll
     for (int l = 0; l < 6; ++l) w_s[l] = s_wimg + lay.w_off[l];
@@ -334,11 +330,12 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     }
 
     // One MMA round: publish the A operand this thread just wrote, let the leader issue, wait for completion.
-    auto mma_round = [&](uint32_t a_d, int layer, int K, int N) {
+    auto publish = [&]() {
         tmem_wait_st();
         tc_fence_before();
         named_bar_sync(1 + wg, 128);
-        if (leader) issue_layer<kBf16>(acc_d, a_d, w_s[layer], K, N, mma_bar);
+    };
+    auto await_mma = [&]() {
         mbar_wait(mma_bar, mma_phase);
         mma_phase ^= 1u;
         tc_fence_after();
@@ -411,34 +408,35 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 x[4 * i] = z4.x; x[4 * i + 1] = z4.y; x[4 * i + 2] = z4.z; x[4 * i + 3] = z4.w;
             }
             x[L / 2] = pack2<kBf16, false>(a.up, a.vp);
-            x[L / 2 + 1] = pack2<kBf16, false>(a.lf, 0.0f);
+            x[L / 2 + 1] = pack2<kBf16, false>(a.lf, tc_bias_const(kBf16, 0));
+            x[L / 2 + 2] = pack2<kBf16, false>(tc_bias_const(kBf16, 1), tc_bias_const(kBf16, 2));
 #pragma unroll
-            for (int i = L / 2 + 2; i < T::K1p / 2; ++i) x[i] = 0u;
+            for (int i = L / 2 + 3; i < T::K1p / 2; ++i) x[i] = 0u;
 #pragma unroll
             for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
         }
 
         // ---- MLP-A (B1-B3) ----
-        tmem_wait_st();
-        tc_fence_before();
-        named_bar_sync(1 + wg, 128);          // every thread has consumed its staged record and stored x
+        publish();                            // every thread has consumed its staged record and stored x
         if (leader) {
             const int64_t next = tile + stride;
             if (tile_is_bulk(next)) {          // stream the next tile's records in while this one computes
                 mbar_expect_tx(q_bar, T::kStageBytes);
                 bulk_g2s(my_stage, q + next * 128, T::kStageBytes, q_bar);
             }
-            issue_layer<kBf16>(acc_d, ay_d, w_s[0], T::K1p, H, mma_bar);
+            issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
         }
-        mbar_wait(mma_bar, mma_phase);
-        mma_phase ^= 1u;
-        tc_fence_after();
+        await_mma();
 
-        epilogue_to_a<H, true, kBf16>(acc_t, ah_t, bias[0]);
-        mma_round(ah_d, 1, H, H);
-        epilogue_to_a<H, true, kBf16>(acc_t, ah_t, bias[1]);
-        mma_round(ah_d, 2, H, kFeat);
-        epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t, bias[2]);      // feat (linear) -> AY columns [0, 16)
+        epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
+        publish();
+        if (leader) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[1], mma_bar);
+        await_mma();
+        epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
+        publish();
+        if (leader) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
+        await_mma();
+        epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t);      // feat (linear) -> AY columns [0, 16)
 
         // ---- MLP-B (B4-B7), once per query / once per light (C1-C3) ----
         float rad[3] = { 0.0f, 0.0f, 0.0f };
@@ -456,20 +454,28 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             y[0] = pack2<kBf16, false>(a.wi[0], a.wi[1]);
             y[1] = pack2<kBf16, false>(a.wi[2], a.wo[0]);
             y[2] = pack2<kBf16, false>(a.wo[1], a.wo[2]);
+            y[3] = c01;
+            y[4] = c2z;
 #pragma unroll
-            for (int i = 3; i < 8; ++i) y[i] = 0u;
+            for (int i = 5; i < 8; ++i) y[i] = 0u;
             tmem_st8(ay_t + 16, y);
-            mma_round(ay_d, 3, T::K4p, H);
-            epilogue_to_a<H, true, kBf16>(acc_t, ah_t, bias[3]);
-            mma_round(ah_d, 4, H, H);
-            epilogue_to_a<H, true, kBf16>(acc_t, ah_t, bias[4]);
-            mma_round(ah_d, 5, H, 16);
+            publish();
+            if (leader) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
+            await_mma();
+            epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
+            publish();
+            if (leader) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+            await_mma();
+            epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
+            publish();
+            if (leader) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[5], mma_bar);
+            await_mma();
             uint32_t o[4];
             tmem_ld4(acc_t, o);
             tmem_wait_ld();
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float v = softplus<true>(__uint_as_float(o[c]) + bias[5][c]);
+                const float v = softplus<true>(__uint_as_float(o[c]));
                 rad[c] = kShade ? fmaf(v * E[c], cs, rad[c]) : v;
             }
         }

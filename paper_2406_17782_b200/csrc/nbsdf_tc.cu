@@ -71,6 +71,18 @@ __device__ __forceinline__ void fence_mbar_init()
 {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
+// true in exactly one lane of a fully converged warp; keeps the surrounding code warp-uniform for the compiler,
+// so that MMA operands (TMEM addresses, descriptors) live in uniform registers
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -266,10 +278,10 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStageBytes + NWG * 16u);
 
     const int tid = threadIdx.x;
-    const int wg = tid >> 7;
     const int t = tid & 127;               // row within the tile == TMEM lane
-    const int warp = tid >> 5;
-    const bool leader = t == 0;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // warp-uniform for the compiler
+    const int wg = warp >> 2;
+    const bool issuer = (warp & 3) == 0;   // warp 0 of each warpgroup issues its MMAs and bulk copies (one elected lane)
     const TcLayout lay = tc_layout(L, H);
 
     // ---- prologue: weights image + packed latents -> shared memory, barriers, TMEM ----
@@ -286,11 +298,12 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     }
     const uint32_t mma_bar = s_bars + (uint32_t)wg * 16u;
     const uint32_t q_bar = mma_bar + 8u;
-    if (leader) {
+    if (issuer && elect_one()) {
         mbar_init(mma_bar, 1);
         mbar_init(q_bar, 1);
         fence_mbar_init();
     }
+    __syncwarp();
     if (warp == 0) {
         tmem_alloc(s_tmem, 512);
         tmem_relinquish();
@@ -298,7 +311,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *g_tmem;
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *g_tmem, 0);
     const uint32_t col0 = tmem_base + (uint32_t)(wg * T::kColsPerWg);                 // lane 0: for MMA operands
     const uint32_t lane_taddr = col0 + ((uint32_t)((warp & 3) * 32) << 16);           // this warp's lane quarter
     const uint32_t acc_t = lane_taddr + T::kAccCol, ah_t = lane_taddr + T::kAhCol, ay_t = lane_taddr + T::kAyCol;
@@ -324,12 +337,13 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStageBytes;
 
     auto tile_is_bulk = [&](int64_t tile) { return !kShade && tile < n_tiles && (tile + 1) * 128 <= n_items; };
-    if (leader && tile_is_bulk(first)) {
+    if (issuer && tile_is_bulk(first) && elect_one()) {
         mbar_expect_tx(q_bar, T::kStageBytes);
         bulk_g2s(my_stage, q + first * 128, T::kStageBytes, q_bar);
     }
+    __syncwarp();
 
-    // One MMA round: publish the A operand this thread just wrote, let the leader issue, wait for completion.
+    // One MMA round: publish the A operand this thread just wrote, let the issuer lane issue, wait for completion.
     auto publish = [&]() {
         tmem_wait_st();
         tc_fence_before();
@@ -418,23 +432,32 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 
         // ---- MLP-A (B1-B3) ----
         publish();                            // every thread has consumed its staged record and stored x
-        if (leader) {
-            const int64_t next = tile + stride;
-            if (tile_is_bulk(next)) {          // stream the next tile's records in while this one computes
-                mbar_expect_tx(q_bar, T::kStageBytes);
-                bulk_g2s(my_stage, q + next * 128, T::kStageBytes, q_bar);
+        if (issuer) {
+            if (elect_one()) {
+                const int64_t next = tile + stride;
+                if (tile_is_bulk(next)) {          // stream the next tile's records in while this one computes
+                    mbar_expect_tx(q_bar, T::kStageBytes);
+                    bulk_g2s(my_stage, q + next * 128, T::kStageBytes, q_bar);
+                }
+                issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
             }
-            issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
+            __syncwarp();
         }
         await_mma();
 
         epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
         publish();
-        if (leader) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[1], mma_bar);
+        if (issuer) {
+            if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[1], mma_bar);
+            __syncwarp();
+        }
         await_mma();
         epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
         publish();
-        if (leader) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
+        if (issuer) {
+            if (elect_one()) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
+            __syncwarp();
+        }
         await_mma();
         epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t);      // feat (linear) -> AY columns [0, 16)
 
@@ -460,15 +483,24 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             for (int i = 5; i < 8; ++i) y[i] = 0u;
             tmem_st8(ay_t + 16, y);
             publish();
-            if (leader) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
+            if (issuer) {
+                if (elect_one()) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
+                __syncwarp();
+            }
             await_mma();
             epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
             publish();
-            if (leader) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+            if (issuer) {
+                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                __syncwarp();
+            }
             await_mma();
             epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
             publish();
-            if (leader) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[5], mma_bar);
+            if (issuer) {
+                if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[5], mma_bar);
+                __syncwarp();
+            }
             await_mma();
             uint32_t o[4];
             tmem_ld4(acc_t, o);

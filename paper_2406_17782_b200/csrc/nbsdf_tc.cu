@@ -83,6 +83,10 @@ __device__ __forceinline__ bool elect_one()
         : "=r"(pred));
     return pred != 0;
 }
+// Programmatic dependent launch: let the next kernel on the stream start its prologue while this one runs, and
+// wait for the previous kernel's memory to be visible before touching anything it may have written.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait_prior_grid() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -285,10 +289,14 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const TcLayout lay = tc_layout(L, H);
 
     // ---- prologue: weights image + packed latents -> shared memory, barriers, TMEM ----
+    // The weight image is immutable after nbsdf_create, so it is fetched before the grid-dependency wait and overlaps
+    // the tail of the previous kernel on the stream; everything a previous kernel or copy may write comes after it.
+    pdl_launch_dependents();
     {
         const uint4* src = reinterpret_cast<const uint4*>(net.wimg);
         uint4* dst = reinterpret_cast<uint4*>(g_wimg);
         for (uint32_t i = tid; i < T::wimg_bytes() / 16u; i += T::kThreads) dst[i] = __ldg(src + i);
+        pdl_wait_prior_grid();
         uint16_t* lat = reinterpret_cast<uint16_t*>(g_lat);
         for (int i = tid; i < net.M * L; i += T::kThreads) {
             const float z = __ldg(net.latents + i);
@@ -539,8 +547,17 @@ static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_que
     int64_t grid = (tiles + NWG - 1) / NWG;
     if (grid > num_sms) grid = num_sms;
     if (grid < 1) grid = 1;
-    kern<<<(unsigned)grid, NWG * 128, T::smem_bytes(), s>>>(net, q, frames, n, fr, lights, out);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(NWG * 128);
+    cfg.dynamicSmemBytes = T::smem_bytes();
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // overlap our prologue with the previous kernel's tail
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, net, q, frames, n, fr, lights, out);
 }
 
 template <bool kShade>

@@ -235,9 +235,12 @@ def run_ours(args):
         us_per_launch = 1e3 * ms / K
         achieved_tf = FLOP_PER_QUERY * n / (us_per_launch * 1e-6) / 1e12
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")      # dram bytes/launch copied from the ncu --set full summary
         if os.path.exists(tp):
-            traffic = json.load(open(tp)).get(f"eval_{prec}_dram_bytes_per_launch")
+            for ln in open(tp).read().splitlines()[1:]:
+                parts = ln.split(",")
+                if parts[0] == f"eval_{prec}_dram_bytes_per_launch":
+                    traffic = int(parts[1])
         frame_flop = npx * (FLOP_MLP_A + 5 * FLOP_MLP_B)
         frame_tf = frame_flop / (fms * 1e-3) / 1e12
         cores = len(os.sched_getaffinity(0))

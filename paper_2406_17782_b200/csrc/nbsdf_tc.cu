@@ -22,6 +22,13 @@
 
 #include "nbsdf_common.cuh"
 
+#ifndef NBSDF_EPI_CHUNK
+#define NBSDF_EPI_CHUNK 32
+#endif
+#ifndef NBSDF_NWG64_EVAL
+#define NBSDF_NWG64_EVAL 4
+#endif
+
 namespace nbsdf {
 
 // ------------------------------------------------------------------------------------------------
@@ -137,6 +144,15 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
           "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
         : "r"(taddr) : "memory");
 }
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr) : "memory");
+}
 __device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4])
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
@@ -194,20 +210,23 @@ __host__ __device__ constexpr uint32_t make_idesc(int N)
 }
 
 // ------------------------------------------------------------------------------------------------
-template <int L, int H, bool kBf16, int NWG>
+template <int L, int H, bool kBf16, int NWG, bool kShade>
 struct Tc {
     static constexpr TcLayout kLay = tc_layout(L, H);
     static constexpr int K1p = kLay.K1p;
     static constexpr int K4p = kLay.K4p;
     static constexpr int kThreads = NWG * 128;
-    static constexpr int kColsPerWg = 512 / NWG;
+    // TMEM columns of one warpgroup.  eval: x, the hidden activations and y share ONE A-operand region (each is dead
+    // before the next is written); shade: y = [feat, wi, wo] must survive the light loop, so it gets its own region.
+    static constexpr int kAw = kShade ? H / 2 : (H / 2 > 24 ? H / 2 : 24);
     static constexpr int kAccCol = 0;
-    static constexpr int kAhCol = H;                 // hidden activations, H/2 columns
-    static constexpr int kOneCol = H + H / 2;        // constant block (c0, c1, c2, 0...): the bias K step of the K = H layers
-    static constexpr int kAyCol = kOneCol + 8;       // x = [z, u', v', lf, c] and later y = [feat, wi, wo, c]
-    static_assert(kAyCol + 24 <= kColsPerWg, "TMEM budget per warpgroup");
+    static constexpr int kAhCol = H;
+    static constexpr int kAyCol = kShade ? H + H / 2 : H;
+    static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw;
+    static constexpr int kOneCol = 504;              // CTA-wide constant block (c0, c1, c2, 0...): bias K step of the K = H layers
+    static_assert(NWG * kColsPerWg <= kOneCol, "TMEM budget");
     static_assert(L % 8 == 0 && H % 32 == 0, "dims");
-    static_assert(K1p <= 48 && K4p == 48, "AY holds at most 24 columns");
+    static_assert(K1p <= 48 && K4p == 48, "x / y hold at most 24 columns");
 
     static constexpr uint32_t kLatBytes = 64 * 32 * 2;            // packed latent table, max M x max L
     static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);
@@ -238,9 +257,23 @@ __device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t a_tmem, ui
 }
 
 // Epilogue of a hidden layer: acc (N fp32 columns, bias already inside) -> (ReLU) -> packed 16-bit pairs -> A columns.
+// 64 columns are fetched per wait so that two tcgen05.ld are in flight.
 template <int N, bool kRelu, bool kBf16>
 __device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_taddr)
 {
+#if NBSDF_EPI_CHUNK == 16
+#pragma unroll
+    for (int c = 0; c < N; c += 16) {
+        uint32_t v[16];
+        tmem_ld16(acc_taddr + c, v);
+        tmem_wait_ld();
+        uint32_t p[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
+        tmem_st8(a_taddr + c / 2, p);
+    }
+#else
 #pragma unroll
     for (int c = 0; c < N; c += 32) {
         uint32_t v[32];
@@ -252,6 +285,7 @@ __device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_tad
             p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
         tmem_st16(a_taddr + c / 2, p);
     }
+#endif
 }
 
 // Per-thread record after input assembly (stages A1-A4)
@@ -266,7 +300,7 @@ __global__ void __launch_bounds__(NWG * 128, 1)
 tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restrict__ frames, int64_t n,
           FrameParams fr, LightParams lights, float* __restrict__ out)
 {
-    using T = Tc<L, H, kBf16, NWG>;
+    using T = Tc<L, H, kBf16, NWG, kShade>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* gbase = smem_raw + (base - smem_u32(smem_raw));
@@ -292,20 +326,21 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     // The weight image is immutable after nbsdf_create, so it is fetched before the grid-dependency wait and overlaps
     // the tail of the previous kernel on the stream; everything a previous kernel or copy may write comes after it.
     pdl_launch_dependents();
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(net.wimg);
-        uint4* dst = reinterpret_cast<uint4*>(g_wimg);
-        for (uint32_t i = tid; i < T::wimg_bytes() / 16u; i += T::kThreads) dst[i] = __ldg(src + i);
-        pdl_wait_prior_grid();
-        uint16_t* lat = reinterpret_cast<uint16_t*>(g_lat);
-        for (int i = tid; i < net.M * L; i += T::kThreads) {
-            const float z = __ldg(net.latents + i);
-            lat[i] = kBf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(z)) : __half_as_ushort(__float2half_rn(z));
-        }
-        fence_proxy_async();   // generic-proxy writes of the weight tiles must be visible to the tensor core (async proxy)
-    }
     const uint32_t mma_bar = s_bars + (uint32_t)wg * 16u;
     const uint32_t q_bar = mma_bar + 8u;
+    const uint32_t w_bar = s_tmem + 8u;
+    if (warp == 0 && elect_one()) {
+        mbar_init(w_bar, 1);
+        fence_mbar_init();
+        // one elected lane streams the whole image in with bulk copies; only the MMA issuers ever wait for it
+        mbar_expect_tx(w_bar, T::wimg_bytes());
+        constexpr uint32_t kChunk = 32768u;
+        for (uint32_t off = 0; off < T::wimg_bytes(); off += kChunk) {
+            const uint32_t bytes = T::wimg_bytes() - off < kChunk ? T::wimg_bytes() - off : kChunk;
+            bulk_g2s(s_wimg + off, net.wimg + off, bytes, w_bar);
+        }
+    }
+    __syncwarp();
     if (issuer && elect_one()) {
         mbar_init(mma_bar, 1);
         mbar_init(q_bar, 1);
@@ -316,22 +351,35 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         tmem_alloc(s_tmem, 512);
         tmem_relinquish();
     }
+    pdl_wait_prior_grid();
+    {
+        uint16_t* lat = reinterpret_cast<uint16_t*>(g_lat);
+        for (int i = tid; i < net.M * L; i += T::kThreads) {
+            const float z = __ldg(net.latents + i);
+            lat[i] = kBf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(z)) : __half_as_ushort(__float2half_rn(z));
+        }
+    }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *g_tmem, 0);
     const uint32_t col0 = tmem_base + (uint32_t)(wg * T::kColsPerWg);                 // lane 0: for MMA operands
-    const uint32_t lane_taddr = col0 + ((uint32_t)((warp & 3) * 32) << 16);           // this warp's lane quarter
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;                      // this warp's lane quarter
+    const uint32_t lane_taddr = col0 + lane_off;
     const uint32_t acc_t = lane_taddr + T::kAccCol, ah_t = lane_taddr + T::kAhCol, ay_t = lane_taddr + T::kAyCol;
-    const uint32_t acc_d = col0 + T::kAccCol, ah_d = col0 + T::kAhCol, ay_d = col0 + T::kAyCol, one_d = col0 + T::kOneCol;
+    const uint32_t acc_d = col0 + T::kAccCol, ah_d = col0 + T::kAhCol, ay_d = col0 + T::kAyCol, one_d = tmem_base + T::kOneCol;
 
-    // bias constants (c0, c1, c2) as packed pairs; the constant block is written once per kernel
+    // bias constants (c0, c1, c2) as packed pairs; the CTA-wide constant block is written once per kernel by warpgroup 0
     const uint32_t c01 = pack2<kBf16, false>(tc_bias_const(kBf16, 0), tc_bias_const(kBf16, 1));
     const uint32_t c2z = pack2<kBf16, false>(tc_bias_const(kBf16, 2), 0.0f);
-    {
+    if (wg == 0) {
         uint32_t ones[8] = { c01, c2z, 0u, 0u, 0u, 0u, 0u, 0u };
-        tmem_st8(lane_taddr + T::kOneCol, ones);
+        tmem_st8(tmem_base + lane_off + T::kOneCol, ones);
+        tmem_wait_st();
     }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
     uint32_t w_s[6];
 #pragma unroll
     for (int l = 0; l < 6; ++l) w_s[l] = s_wimg + lay.w_off[l];
@@ -341,6 +389,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const int64_t stride = (int64_t)gridDim.x * NWG;
     const int64_t first = (int64_t)blockIdx.x * NWG + wg;
     uint32_t mma_phase = 0, q_phase = 0;
+    bool weights_ready = false;
     const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStageBytes;
     const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStageBytes;
 
@@ -447,8 +496,10 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                     mbar_expect_tx(q_bar, T::kStageBytes);
                     bulk_g2s(my_stage, q + next * 128, T::kStageBytes, q_bar);
                 }
+                if (!weights_ready) mbar_wait(w_bar, 0);
                 issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
             }
+            weights_ready = true;
             __syncwarp();
         }
         await_mma();
@@ -538,8 +589,8 @@ template <int L, int H, bool kBf16, bool kShade>
 static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_query* q, const float* frames, int64_t n,
                               const FrameParams& fr, const LightParams& lights, float* out, cudaStream_t s, bool init_only)
 {
-    constexpr int NWG = H == 128 ? 2 : 4;
-    using T = Tc<L, H, kBf16, NWG>;
+    constexpr int NWG = H == 128 ? 2 : (H == 32 ? 6 : (kShade ? 4 : NBSDF_NWG64_EVAL));
+    using T = Tc<L, H, kBf16, NWG, kShade>;
     auto kern = tc_kernel<L, H, kBf16, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());
     const int64_t n_items = kShade ? fr.n_pixels : n;

@@ -282,6 +282,53 @@ def run_ours(args):
         print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: N in 2^12..2^26 (x4 steps) x H in {32,64,128} x L in {8,16,32}, 8 materials, seed per
+    point.  One JSON line per point: queries/s, binding roofline and fraction, oracle parity on min(N, 2^16) leading
+    queries.  Not the headline line; `python bench.py --sweep > profiles/...` regenerates the committed table."""
+    import torch
+    import oracle
+    from paper_2406_17782_b200 import api, synth
+    torch.cuda.set_device(0)
+    peaks = measured_peaks()
+    prec = args.precision
+    Ns = [1 << e for e in range(12, 27, 2)]
+    if args.sweep_max_log2 < 26:
+        Ns = [n for n in Ns if n <= (1 << args.sweep_max_log2)]
+    for i_h, H in enumerate((32, 64, 128)):
+        for i_l, L in enumerate((8, 16, 32)):
+            flop = 2 * ((L + 3) * H + H * H + H * 32 + 38 * H + H * H + 3 * H)
+            t_tensor = flop / (peaks["bf16_tflops"] * 1e12)
+            t_hbm = BYTES_PER_QUERY / (peaks["hbm_gbs"] * 1e9)
+            bound = "tensor" if t_tensor >= t_hbm else "hbm"
+            for i_n, n in enumerate(Ns):
+                cfg = synth.config(4, n=n, L=L, H=H, seed=synth.sweep_seed(i_n, i_h, i_l))
+                ctx = api.nbsdf_create(cfg["weights"], cfg["biases"], L, H, 8, prec)
+                api.nbsdf_set_latents(ctx, 0, cfg["latents"])
+                n_rot = max(1, min(8, int(400e6 // (n * BYTES_PER_QUERY)) + 1)) if n * BYTES_PER_QUERY < 200e6 else 1
+                qs = [api.queries_to_device(np.roll(cfg["queries"], r * 977)) for r in range(n_rot)]
+                outs = [torch.empty((n, 3), dtype=torch.float32, device="cuda") for _ in range(n_rot)]
+                api.nbsdf_eval(ctx, qs[0], None, n, outs[0])
+                torch.cuda.synchronize()
+                m = min(n, 1 << 16)
+                ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"][:m])
+                rel = np.abs(outs[0][:m].cpu().numpy().astype(np.float64) - ref) / np.maximum(np.abs(ref), 1e-6)
+                k = int(max(10, min(2000, 2e9 / (n * 40))))
+                for i in range(5):
+                    api.nbsdf_eval(ctx, qs[i % n_rot], None, n, outs[i % n_rot])
+                ms = time_loop(torch, lambda i: api.nbsdf_eval(ctx, qs[i % n_rot], None, n, outs[i % n_rot]), k, lambda: None) / k
+                qps = n / (ms * 1e-3)
+                frac = qps * (t_tensor if bound == "tensor" else t_hbm)
+                print(json.dumps({"config": 4, "n": n, "H": H, "L": L, "precision": prec, "us_per_launch": ms * 1e3,
+                                  "queries_per_s": qps, "flop_per_query": flop, "bound": bound, "roofline_frac": frac,
+                                  "tensor_frac": qps * t_tensor, "hbm_frac": qps * t_hbm, "launches_timed": k,
+                                  "rotating_batches": n_rot, "parity_queries": m, "max_rel": float(rel.max()),
+                                  "mean_rel": float(rel.mean())}), flush=True)
+                api.nbsdf_destroy(ctx)
+                del qs, outs
+                torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -289,8 +336,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--precision", default="fp16", choices=["fp16", "bf16", "fp32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--sweep", action="store_true", help="configs[4] scaling sweep instead of the headline line")
+    ap.add_argument("--sweep-max-log2", type=int, default=26)
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

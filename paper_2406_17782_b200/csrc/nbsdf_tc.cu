@@ -25,6 +25,9 @@
 #ifndef NBSDF_EPI_CHUNK
 #define NBSDF_EPI_CHUNK 32
 #endif
+#ifndef NBSDF_NWG32_EVAL
+#define NBSDF_NWG32_EVAL 8
+#endif
 #ifndef NBSDF_NWG64_EVAL
 #define NBSDF_NWG64_EVAL 4
 #endif
@@ -589,7 +592,7 @@ template <int L, int H, bool kBf16, bool kShade>
 static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_query* q, const float* frames, int64_t n,
                               const FrameParams& fr, const LightParams& lights, float* out, cudaStream_t s, bool init_only)
 {
-    constexpr int NWG = H == 128 ? 2 : (H == 32 ? 6 : (kShade ? 4 : NBSDF_NWG64_EVAL));
+    constexpr int NWG = H == 128 ? 2 : (H == 32 ? (kShade ? 6 : NBSDF_NWG32_EVAL) : (kShade ? 4 : NBSDF_NWG64_EVAL));
     using T = Tc<L, H, kBf16, NWG, kShade>;
     auto kern = tc_kernel<L, H, kBf16, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());

@@ -78,7 +78,7 @@ class ClockSampler:
                 self.reasons.update(self._reasons())
             except Exception:
                 pass
-            time.sleep(0.004)
+            time.sleep(0.002)
 
     def start(self):
         if self.nv is not None:

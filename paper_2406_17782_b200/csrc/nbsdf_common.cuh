@@ -15,9 +15,9 @@ constexpr int kTileRows = 128;     // queries per tile = TMEM lanes = threads pe
 struct NetParams {
     const float* latents;   // [M][L] fp32 latent table ("material latent vector")
     const float* w32;       // fp32 path: transposed, padded weights + biases (see pack_fp32)
-    const uint8_t* wimg;    // tensor path: shared-memory image (weights as swizzled UMMA tiles, biases)
+    const uint8_t* wimg_eval;    // tensor path: shared-memory image for nbsdf_eval (5 layers, feature layer merged)
+    const uint8_t* wimg_shade;   // tensor path: shared-memory image for nbsdf_shade_frame (6 layers)
     int32_t L, H, M;
-    uint32_t wimg_bytes;
 };
 
 struct LightParams {
@@ -149,6 +149,7 @@ __host__ __device__ constexpr float tc_bias_const(bool bf16, int j)
 }
 
 struct TcLayout {
+    int n_layers;            // 6, or 5 when the linear feature layer is merged into layer 4 (eval image)
     int K1p, K4p;            // padded K of layers 1 and 4 (multiples of 16), bias columns included
     int Kp[6];               // padded K of every layer as issued (K = H layers: H + 16)
     int Kbias[6];            // input index of the first bias column of every layer
@@ -159,21 +160,36 @@ struct TcLayout {
 
 __host__ __device__ constexpr int pad16(int k) { return (k + 15) & ~15; }
 
-__host__ __device__ constexpr TcLayout tc_layout(int L, int H)
+// merged == false: the six layers as defined (nbsdf_shade_frame, where the feature is reused across lights; and H = 128).
+// merged == true : nbsdf_eval's image for H <= 64.  The feature layer is linear, so
+//                  W4[:, :F] (W3 h2 + b3) + W4[:, F:] [wi, wo] + b4 == (W4f W3) h2 + W4a [wi, wo] + (W4f b3 + b4):
+//                  layers 3 and 4 become ONE H x (H + 6) layer, one MMA round and one epilogue fewer per tile.
+//                  Multiply-adds: H (H + 6) merged vs 2 F H + 6 H separate -- equal at H = 64 (F = 32), fewer at H = 32,
+//                  twice as many at H = 128 (which is why H = 128 keeps six layers).  Its last K step reads
+//                  [wi, wo, c0, c1, c2] from a per-warpgroup tail block instead of the CTA-wide bias-constant block.
+__host__ __device__ constexpr bool tc_eval_merged(int H) { return H <= 64; }
+
+__host__ __device__ constexpr TcLayout tc_layout(int L, int H, bool merged)
 {
     TcLayout t{};
     t.K1p = pad16(L + 3 + kBiasCols);
     t.K4p = pad16(kFeat + 6 + kBiasCols);
-    const int K[6] = { t.K1p, H + 16, H + 16, t.K4p, H + 16, H + 16 };
-    const int Kb[6] = { L + 3, H, H, kFeat + 6, H, H };
-    const int N[6] = { H, H, kFeat, H, H, 16 };
+    t.n_layers = merged ? 5 : 6;
+    const int K6[6] = { t.K1p, H + 16, H + 16, t.K4p, H + 16, H + 16 };
+    const int Kb6[6] = { L + 3, H, H, kFeat + 6, H, H };
+    const int N6[6] = { H, H, kFeat, H, H, 16 };
+    const int K5[6] = { t.K1p, H + 16, H + 16, H + 16, H + 16, 0 };
+    const int Kb5[6] = { L + 3, H, H + 6, H, H, 0 };
+    const int N5[6] = { H, H, H, H, 16, 0 };
     uint32_t off = 0;
-    for (int l = 0; l < 6; ++l) {
-        t.Kp[l] = K[l];
-        t.Kbias[l] = Kb[l];
+    for (int l = 0; l < t.n_layers; ++l) {
+        const int K = merged ? K5[l] : K6[l];
+        const int N = merged ? N5[l] : N6[l];
+        t.Kp[l] = K;
+        t.Kbias[l] = merged ? Kb5[l] : Kb6[l];
         t.w_off[l] = off;
-        t.w_rows[l] = (uint32_t)N[l];
-        off += (uint32_t)((K[l] + 63) / 64) * (uint32_t)N[l] * 128u;   // N rows x 128 B per 64-wide K block
+        t.w_rows[l] = (uint32_t)N;
+        off += (uint32_t)((K + 63) / 64) * (uint32_t)N * 128u;   // N rows x 128 B per 64-wide K block
     }
     t.total = (off + 15u) & ~15u;
     return t;

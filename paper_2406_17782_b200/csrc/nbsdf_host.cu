@@ -23,8 +23,8 @@ struct nbsdf_ctx {
     int num_sms = 0;
     float* d_latents = nullptr;       // [M][L] fp32
     float* d_w32 = nullptr;           // fp32 path blob
-    uint8_t* d_wimg = nullptr;        // tensor path shared-memory image
-    uint32_t wimg_bytes = 0;
+    uint8_t* d_wimg_eval = nullptr;   // tensor path shared-memory images (see tc_layout)
+    uint8_t* d_wimg_shade = nullptr;
     float* h_stage = nullptr;         // pinned mirror used by set_latents
     cudaEvent_t stage_free = nullptr; // recorded after the last staged copy
     bool stage_busy = false;
@@ -62,11 +62,13 @@ static float from_op16(uint16_t bits, bool bf16)
 // 16-byte chunk index XOR-ed by (row % 8) (the 128-byte swizzle tcgen05 applies when it reads the tile).
 // Columns [Kbias, Kbias + 3) of every row hold the three-way 16-bit split of the fp32 bias, each part divided by
 // the constant the kernel feeds in that input column (tc_bias_const), so that sum_j w_j * c_j == bias to ~2^-24.
-static void pack_tc(int L, int H, bool bf16, const nbsdf_weights* w, uint8_t* img)
+// merged: layers 3 and 4 are multiplied out in double (the feature layer is linear, see tc_layout).
+static void pack_tc(int L, int H, bool bf16, bool merged, const nbsdf_weights* w, uint8_t* img)
 {
-    const TcLayout lay = tc_layout(L, H);
-    const int Kr[6] = { L + 3, H, H, kFeat + 6, H, H };
-    const int Nr[6] = { H, H, kFeat, H, H, 3 };
+    const TcLayout lay = tc_layout(L, H, merged);
+    const int F = kFeat;
+    const int Kr6[6] = { L + 3, H, H, F + 6, H, H };
+    const int Nr6[6] = { H, H, F, H, H, 3 };
     memset(img, 0, lay.total);
     auto put = [&](int l, int n, int k, uint16_t bits) {
         const int Np = (int)lay.w_rows[l];
@@ -75,17 +77,37 @@ static void pack_tc(int L, int H, bool bf16, const nbsdf_weights* w, uint8_t* im
         const size_t off = lay.w_off[l] + (size_t)kb * Np * 128 + (size_t)n * 128 + (size_t)chunk * 16 + (size_t)(kk % 8) * 2;
         memcpy(img + off, &bits, 2);
     };
+    auto put_bias = [&](int l, int n, double b) {
+        double r = b;
+        for (int j = 0; j < kBiasCols; ++j) {
+            const double c = (double)tc_bias_const(bf16, j);
+            const uint16_t bits = to_op16((float)(r / c), bf16);
+            put(l, n, lay.Kbias[l] + j, bits);
+            r -= (double)from_op16(bits, bf16) * c;
+        }
+    };
+    int dst = 0;
     for (int l = 0; l < 6; ++l) {
-        for (int n = 0; n < Nr[l]; ++n) {
-            for (int k = 0; k < Kr[l]; ++k) put(l, n, k, to_op16(w->W[l][(size_t)n * Kr[l] + k], bf16));
-            double r = (double)w->b[l][n];
-            for (int j = 0; j < kBiasCols; ++j) {
-                const double c = (double)tc_bias_const(bf16, j);
-                const uint16_t bits = to_op16((float)(r / c), bf16);
-                put(l, n, lay.Kbias[l] + j, bits);
-                r -= (double)from_op16(bits, bf16) * c;
+        if (merged && l == 2) continue;          // folded into layer 4 below
+        if (merged && l == 3) {
+            for (int n = 0; n < H; ++n) {
+                for (int k = 0; k < H; ++k) {
+                    double acc = 0.0;
+                    for (int j = 0; j < F; ++j) acc += (double)w->W[3][(size_t)n * (F + 6) + j] * (double)w->W[2][(size_t)j * H + k];
+                    put(dst, n, k, to_op16((float)acc, bf16));
+                }
+                for (int i = 0; i < 6; ++i) put(dst, n, H + i, to_op16(w->W[3][(size_t)n * (F + 6) + F + i], bf16));
+                double b = (double)w->b[3][n];
+                for (int j = 0; j < F; ++j) b += (double)w->W[3][(size_t)n * (F + 6) + j] * (double)w->b[2][j];
+                put_bias(dst, n, b);
+            }
+        } else {
+            for (int n = 0; n < Nr6[l]; ++n) {
+                for (int k = 0; k < Kr6[l]; ++k) put(dst, n, k, to_op16(w->W[l][(size_t)n * Kr6[l] + k], bf16));
+                put_bias(dst, n, (double)w->b[l][n]);
             }
         }
+        ++dst;
     }
 }
 
@@ -146,12 +168,15 @@ extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weight
         NBSDF_TRY(cudaMemcpy(ctx->d_w32, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(w32)");
         NBSDF_TRY(init_fp32(), "cudaFuncSetAttribute(fp32)");
     } else {
-        const TcLayout lay = tc_layout(L, H);
-        std::vector<uint8_t> img(lay.total);
-        pack_tc(L, H, cfg->precision == NBSDF_PREC_BF16, weights, img.data());
-        ctx->wimg_bytes = lay.total;
-        NBSDF_TRY(cudaMalloc(&ctx->d_wimg, lay.total), "cudaMalloc(wimg)");
-        NBSDF_TRY(cudaMemcpy(ctx->d_wimg, img.data(), lay.total, cudaMemcpyHostToDevice), "cudaMemcpy(wimg)");
+        for (int which = 0; which < 2; ++which) {          // 0: shade image, 1: eval image
+            const bool merged = which == 1 && tc_eval_merged(H);
+            const TcLayout lay = tc_layout(L, H, merged);
+            std::vector<uint8_t> img(lay.total);
+            pack_tc(L, H, cfg->precision == NBSDF_PREC_BF16, merged, weights, img.data());
+            uint8_t** dst = which ? &ctx->d_wimg_eval : &ctx->d_wimg_shade;
+            NBSDF_TRY(cudaMalloc(dst, lay.total), "cudaMalloc(wimg)");
+            NBSDF_TRY(cudaMemcpy(*dst, img.data(), lay.total, cudaMemcpyHostToDevice), "cudaMemcpy(wimg)");
+        }
         NBSDF_TRY(init_tc(L, H), "cudaFuncSetAttribute(tc)");
     }
 #undef NBSDF_TRY
@@ -165,7 +190,8 @@ extern "C" void nbsdf_destroy(nbsdf_ctx* ctx)
     if (ctx->stage_busy && ctx->stage_free) cudaEventSynchronize(ctx->stage_free);
     if (ctx->d_latents) cudaFree(ctx->d_latents);
     if (ctx->d_w32) cudaFree(ctx->d_w32);
-    if (ctx->d_wimg) cudaFree(ctx->d_wimg);
+    if (ctx->d_wimg_eval) cudaFree(ctx->d_wimg_eval);
+    if (ctx->d_wimg_shade) cudaFree(ctx->d_wimg_shade);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->stage_free) cudaEventDestroy(ctx->stage_free);
     delete ctx;
@@ -210,11 +236,11 @@ static NetParams net_params(const nbsdf_ctx* ctx)
     NetParams p;
     p.latents = ctx->d_latents;
     p.w32 = ctx->d_w32;
-    p.wimg = ctx->d_wimg;
+    p.wimg_eval = ctx->d_wimg_eval;
+    p.wimg_shade = ctx->d_wimg_shade;
     p.L = ctx->cfg.latent_dim;
     p.H = ctx->cfg.hidden;
     p.M = ctx->cfg.max_materials;
-    p.wimg_bytes = ctx->wimg_bytes;
     return p;
 }
 

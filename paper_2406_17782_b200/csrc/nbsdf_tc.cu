@@ -26,7 +26,7 @@
 #define NBSDF_EPI_CHUNK 32
 #endif
 #ifndef NBSDF_NWG32_EVAL
-#define NBSDF_NWG32_EVAL 8
+#define NBSDF_NWG32_EVAL 7
 #endif
 #ifndef NBSDF_NWG64_EVAL
 #define NBSDF_NWG64_EVAL 4
@@ -215,17 +215,20 @@ __host__ __device__ constexpr uint32_t make_idesc(int N)
 // ------------------------------------------------------------------------------------------------
 template <int L, int H, bool kBf16, int NWG, bool kShade>
 struct Tc {
-    static constexpr TcLayout kLay = tc_layout(L, H);
+    static constexpr bool kMerged = !kShade && tc_eval_merged(H);    // eval, H <= 64: layers 3 and 4 are one layer
+    static constexpr TcLayout kLay = tc_layout(L, H, kMerged);
     static constexpr int K1p = kLay.K1p;
     static constexpr int K4p = kLay.K4p;
     static constexpr int kThreads = NWG * 128;
     // TMEM columns of one warpgroup.  eval: x, the hidden activations and y share ONE A-operand region (each is dead
     // before the next is written); shade: y = [feat, wi, wo] must survive the light loop, so it gets its own region.
+    // Merged eval adds an 8-column tail block [wi, wo, c0, c1, c2, 0...]: the last K step of the merged layer.
     static constexpr int kAw = kShade ? H / 2 : (H / 2 > 24 ? H / 2 : 24);
     static constexpr int kAccCol = 0;
     static constexpr int kAhCol = H;
     static constexpr int kAyCol = kShade ? H + H / 2 : H;
-    static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw;
+    static constexpr int kTailCol = H + kAw;
+    static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw + (kMerged ? 8 : 0);
     static constexpr int kOneCol = 504;              // CTA-wide constant block (c0, c1, c2, 0...): bias K step of the K = H layers
     static_assert(NWG * kColsPerWg <= kOneCol, "TMEM budget");
     static_assert(L % 8 == 0 && H % 32 == 0, "dims");
@@ -323,7 +326,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // warp-uniform for the compiler
     const int wg = warp >> 2;
     const bool issuer = (warp & 3) == 0;   // warp 0 of each warpgroup issues its MMAs and bulk copies (one elected lane)
-    const TcLayout lay = tc_layout(L, H);
+    constexpr TcLayout lay = T::kLay;
 
     // ---- prologue: weights image + packed latents -> shared memory, barriers, TMEM ----
     // The weight image is immutable after nbsdf_create, so it is fetched before the grid-dependency wait and overlaps
@@ -340,7 +343,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         constexpr uint32_t kChunk = 32768u;
         for (uint32_t off = 0; off < T::wimg_bytes(); off += kChunk) {
             const uint32_t bytes = T::wimg_bytes() - off < kChunk ? T::wimg_bytes() - off : kChunk;
-            bulk_g2s(s_wimg + off, net.wimg + off, bytes, w_bar);
+            bulk_g2s(s_wimg + off, (kShade ? net.wimg_shade : net.wimg_eval) + off, bytes, w_bar);
         }
     }
     __syncwarp();
@@ -385,7 +388,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     tc_fence_after();
     uint32_t w_s[6];
 #pragma unroll
-    for (int l = 0; l < 6; ++l) w_s[l] = s_wimg + lay.w_off[l];
+    for (int l = 0; l < 6; ++l) w_s[l] = s_wimg + (l < lay.n_layers ? lay.w_off[l] : 0u);
 
     const int64_t n_items = kShade ? fr.n_pixels : n;
     const int64_t n_tiles = (n_items + 127) / 128;
@@ -488,6 +491,17 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             for (int i = L / 2 + 3; i < T::K1p / 2; ++i) x[i] = 0u;
 #pragma unroll
             for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
+            if constexpr (T::kMerged) {   // tail block of the merged layer: [wi, wo, c0, c1, c2, 0...]
+                uint32_t y[8];
+                y[0] = pack2<kBf16, false>(a.wi[0], a.wi[1]);
+                y[1] = pack2<kBf16, false>(a.wi[2], a.wo[0]);
+                y[2] = pack2<kBf16, false>(a.wo[1], a.wo[2]);
+                y[3] = c01;
+                y[4] = c2z;
+#pragma unroll
+                for (int i = 5; i < 8; ++i) y[i] = 0u;
+                tmem_st8(lane_taddr + T::kTailCol, y);
+            }
         }
 
         // ---- MLP-A (B1-B3) ----
@@ -515,52 +529,18 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         }
         await_mma();
         epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-        publish();
-        if (issuer) {
-            if (elect_one()) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
-            __syncwarp();
-        }
-        await_mma();
-        epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t);      // feat (linear) -> AY columns [0, 16)
-
-        // ---- MLP-B (B4-B7), once per query / once per light (C1-C3) ----
         float rad[3] = { 0.0f, 0.0f, 0.0f };
-        const int n_rounds = kShade ? lights.n : 1;
-        for (int l = 0; l < n_rounds; ++l) {
-            float E[3] = { 1.0f, 1.0f, 1.0f };
-            float cs = 1.0f;
-            if (kShade) {
-                float wiw[3];
-                light_sample(lights.light[l], px, py, pz, wiw, E);
-                to_local(f, wiw[0], wiw[1], wiw[2], a.wi);
-                cs = fmaxf(a.wi[2], 0.0f);
-            }
-            uint32_t y[8];
-            y[0] = pack2<kBf16, false>(a.wi[0], a.wi[1]);
-            y[1] = pack2<kBf16, false>(a.wi[2], a.wo[0]);
-            y[2] = pack2<kBf16, false>(a.wo[1], a.wo[2]);
-            y[3] = c01;
-            y[4] = c2z;
-#pragma unroll
-            for (int i = 5; i < 8; ++i) y[i] = 0u;
-            tmem_st8(ay_t + 16, y);
-            publish();
+        // last two layers of MLP-B + softplus (B5-B7); g1 has just been published as the A operand
+        auto finish_mlp_b = [&](uint32_t w5, uint32_t w6, const float E[3], float cs) {
             if (issuer) {
-                if (elect_one()) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
+                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w5, mma_bar);
                 __syncwarp();
             }
             await_mma();
             epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
             publish();
             if (issuer) {
-                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
-                __syncwarp();
-            }
-            await_mma();
-            epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-            publish();
-            if (issuer) {
-                if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[5], mma_bar);
+                if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w6, mma_bar);
                 __syncwarp();
             }
             await_mma();
@@ -571,6 +551,58 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             for (int c = 0; c < 3; ++c) {
                 const float v = softplus<true>(__uint_as_float(o[c]));
                 rad[c] = kShade ? fmaf(v * E[c], cs, rad[c]) : v;
+            }
+        };
+        if constexpr (T::kMerged) {
+            // ---- merged layers 3+4 (B3-B4): (W4f W3) h2 + W4a [wi, wo] + (W4f b3 + b4); K = H from AH + tail block ----
+            publish();
+            if (issuer) {
+                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, col0 + T::kTailCol, w_s[2], mma_bar);
+                __syncwarp();
+            }
+            await_mma();
+            epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
+            publish();
+            const float E1[3] = { 1.0f, 1.0f, 1.0f };
+            finish_mlp_b(w_s[3], w_s[4], E1, 1.0f);
+        } else {
+            publish();
+            if (issuer) {
+                if (elect_one()) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
+                __syncwarp();
+            }
+            await_mma();
+            epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t);      // feat (linear) -> AY columns [0, 16)
+
+            // ---- MLP-B (B4-B7), once per query / once per light (C1-C3) ----
+            const int n_rounds = kShade ? lights.n : 1;
+            for (int l = 0; l < n_rounds; ++l) {
+                float E[3] = { 1.0f, 1.0f, 1.0f };
+                float cs = 1.0f;
+                if (kShade) {
+                    float wiw[3];
+                    light_sample(lights.light[l], px, py, pz, wiw, E);
+                    to_local(f, wiw[0], wiw[1], wiw[2], a.wi);
+                    cs = fmaxf(a.wi[2], 0.0f);
+                }
+                uint32_t y[8];
+                y[0] = pack2<kBf16, false>(a.wi[0], a.wi[1]);
+                y[1] = pack2<kBf16, false>(a.wi[2], a.wo[0]);
+                y[2] = pack2<kBf16, false>(a.wo[1], a.wo[2]);
+                y[3] = c01;
+                y[4] = c2z;
+#pragma unroll
+                for (int i = 5; i < 8; ++i) y[i] = 0u;
+                tmem_st8(ay_t + 16, y);
+                publish();
+                if (issuer) {
+                    if (elect_one()) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
+                    __syncwarp();
+                }
+                await_mma();
+                epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
+                publish();
+                finish_mlp_b(w_s[4], w_s[5], E, cs);
             }
         }
         if (live) {

@@ -31,6 +31,13 @@ def build(force=False):
 
 
 _lib = None
+_all_threads = 1
+
+
+def _threads(n):
+    """0 = all cores the process started with (an earlier 1-thread call must not stick)."""
+    _load()
+    return int(n) if n and n > 0 else _all_threads
 
 
 def _load():
@@ -52,6 +59,8 @@ def _load():
         lib.oracle_shade_frame.argtypes = [C.c_void_p] * 8 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
                                                               C.c_int, C.c_void_p, C.c_int]
         lib.oracle_max_threads.restype = C.c_int
+        global _all_threads
+        _all_threads = int(lib.oracle_max_threads())      # before any call narrows the OpenMP team
         _lib = lib
     return _lib
 
@@ -90,7 +99,7 @@ def eval_queries(weights, biases, latents, queries, frames=None, n_threads=0):
     assert n == 0 or int(mats.max()) < Z.shape[0], "material id out of range"
     out = np.empty((n, 3), dtype=np.float64)
     rc = _load().oracle_eval(C.byref(dims), Wp, bp, Z.ctypes.data, q.ctypes.data,
-                             fr.ctypes.data if fr is not None else None, n, out.ctypes.data, int(n_threads))
+                             fr.ctypes.data if fr is not None else None, n, out.ctypes.data, _threads(n_threads))
     assert rc == 0
     return out
 
@@ -115,7 +124,7 @@ def shade_frame(weights, biases, latents, gbuffer, lights, first=0, count=None, 
     rc = _load().oracle_shade_frame(C.byref(dims), Wp, bp, Z.ctypes.data, pos.ctypes.data, nrm.ctypes.data,
                                     tan.ctypes.data, mat.ctypes.data, first, count, cam.ctypes.data,
                                     lt.ctypes.data if lt.shape[0] else None, lt.shape[0], out.ctypes.data,
-                                    int(n_threads))
+                                    _threads(n_threads))
     assert rc == 0
     return out
 
@@ -142,4 +151,5 @@ def to_local(n, t, w):
 
 
 def max_threads():
-    return int(_load().oracle_max_threads())
+    _load()
+    return _all_threads

@@ -22,17 +22,33 @@
 
 #include "nbsdf_common.cuh"
 
-#ifndef NBSDF_EPI_CHUNK
-#define NBSDF_EPI_CHUNK 32
-#endif
 #ifndef NBSDF_NWG32_EVAL
-#define NBSDF_NWG32_EVAL 7
+#define NBSDF_NWG32_EVAL 6
 #endif
 #ifndef NBSDF_NWG64_EVAL
 #define NBSDF_NWG64_EVAL 4
 #endif
 
 namespace nbsdf {
+
+#ifdef NBSDF_PHASE_PROBE
+// debug builds only: cycles thread 0 of CTA 0 spends in each phase of the merged eval chain (summed over its tiles)
+__device__ long long g_phase_probe[32];
+#define NBSDF_PHASE(i) do { const long long now_ = clock64(); ph_acc[i] += now_ - ph_last; ph_last = now_; } while (0)
+#else
+#define NBSDF_PHASE(i) do { } while (0)
+#endif
+
+#ifdef NBSDF_CLOCK_PROBE
+// debug builds only: SM clock ticks and global-timer nanoseconds at the start and end of CTA 0 of the last launch
+__device__ unsigned long long g_clock_probe[4];
+__device__ __forceinline__ unsigned long long global_timer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -101,6 +117,17 @@ __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+
+__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t nthreads)
+{
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// Moves registers between warpgroups after launch (all four warps of a warpgroup execute the same one)
+template <int kRegs>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
+template <int kRegs>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
 {
@@ -219,7 +246,16 @@ struct Tc {
     static constexpr TcLayout kLay = tc_layout(L, H, kMerged);
     static constexpr int K1p = kLay.K1p;
     static constexpr int K4p = kLay.K4p;
-    static constexpr int kThreads = NWG * 128;
+    // Warps [0, 4 NWG) are the warpgroups that own tile rows; then one MMA-issuer warp per warpgroup, padded to whole
+    // warpgroups so that setmaxnreg can move the issuers' registers to the row owners.
+    static constexpr int kIssuerWarps = (NWG + 3) / 4 * 4;
+    static constexpr int kThreads = NWG * 128 + kIssuerWarps * 32;
+    static constexpr int kIssuerRegs = 56;
+    static constexpr int kBaseRegs = 65536 / kThreads / 8 * 8 > 248 ? 248 : 65536 / kThreads / 8 * 8;      // what ptxas is told
+    // only what the issuer warps give back is available to setmaxnreg.inc (not the register file's unallocated rest)
+    static constexpr int kOwnerRegsRaw = kBaseRegs + kIssuerWarps * 32 * (kBaseRegs - kIssuerRegs) / (NWG * 128) / 8 * 8;
+    static constexpr int kOwnerRegs = kOwnerRegsRaw > 248 ? 248 : kOwnerRegsRaw;
+    static_assert(kThreads <= 1024, "CTA size");
     // TMEM columns of one warpgroup.  eval: x, the hidden activations and y share ONE A-operand region (each is dead
     // before the next is written); shade: y = [feat, wi, wo] must survive the light loop, so it gets its own region.
     // Merged eval adds an 8-column tail block [wi, wo, c0, c1, c2, 0...]: the last K step of the merged layer.
@@ -236,11 +272,13 @@ struct Tc {
 
     static constexpr uint32_t kLatBytes = 64 * 32 * 2;            // packed latent table, max M x max L
     static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);
+    static constexpr uint32_t kStages = 2;                        // staging buffers per warpgroup
+    static constexpr bool kTwoLoads = NWG * 128 * 160 <= 65536 || !kShade;   // epilogue register budget (see epilogue_to_a)
 
     __host__ __device__ static constexpr uint32_t wimg_bytes() { return kLay.total; }
     __host__ __device__ static constexpr uint32_t smem_bytes()
     {
-        return 1024u + ((wimg_bytes() + 127u) & ~127u) + kLatBytes + NWG * kStageBytes + 256u;
+        return 1024u + ((wimg_bytes() + 127u) & ~127u) + kLatBytes + NWG * kStages * kStageBytes + NWG * 32u + 64u;
     }
 };
 
@@ -263,46 +301,55 @@ __device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t a_tmem, ui
 }
 
 // Epilogue of a hidden layer: acc (N fp32 columns, bias already inside) -> (ReLU) -> packed 16-bit pairs -> A columns.
-// 64 columns are fetched per wait so that two tcgen05.ld are in flight.
-template <int N, bool kRelu, bool kBf16>
+// kTwoLoads: 64 columns (two tcgen05.ld) are requested per wait, so the second load's latency hides behind the
+// first's; costs 32 more live registers.
+template <int N, bool kRelu, bool kBf16, bool kTwoLoads = true>
 __device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_taddr)
 {
-#if NBSDF_EPI_CHUNK == 16
+    if constexpr (kTwoLoads && N % 64 == 0) {
 #pragma unroll
-    for (int c = 0; c < N; c += 16) {
-        uint32_t v[16];
-        tmem_ld16(acc_taddr + c, v);
-        tmem_wait_ld();
-        uint32_t p[8];
+        for (int c = 0; c < N; c += 64) {
+            uint32_t v[32], w[32];
+            tmem_ld32(acc_taddr + c, v);
+            tmem_ld32(acc_taddr + c + 32, w);
+            tmem_wait_ld();
+            uint32_t p[16];
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
-            p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
-        tmem_st8(a_taddr + c / 2, p);
+            for (int j = 0; j < 16; ++j)
+                p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
+            tmem_st16(a_taddr + c / 2, p);
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+                p[j] = pack2<kBf16, kRelu>(__uint_as_float(w[2 * j]), __uint_as_float(w[2 * j + 1]));
+            tmem_st16(a_taddr + c / 2 + 16, p);
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < N; c += 32) {
+            uint32_t v[32];
+            tmem_ld32(acc_taddr + c, v);
+            tmem_wait_ld();
+            uint32_t p[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+                p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
+            tmem_st16(a_taddr + c / 2, p);
+        }
     }
-#else
-#pragma unroll
-    for (int c = 0; c < N; c += 32) {
-        uint32_t v[32];
-        tmem_ld32(acc_taddr + c, v);
-        tmem_wait_ld();
-        uint32_t p[16];
-#pragma unroll
-        for (int j = 0; j < 16; ++j)
-            p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
-        tmem_st16(a_taddr + c / 2, p);
-    }
-#endif
 }
 
-// Per-thread record after input assembly (stages A1-A4)
-struct Assembled {
-    float up, vp, lf;
-    float wi[3], wo[3];
-    int material;
-};
-
+// The kernel.  Per warpgroup and 128-row tile the layer chain is strictly sequential
+//   [operand in TMEM] -> warpgroup barrier -> one lane issues the layer's MMAs + commit -> all wait -> epilogue -> ...
+// and a round trip (barrier, issue, commit, wake-up, tcgen05.ld, convert, tcgen05.st) costs about as much as the MMAs
+// themselves, so the tensor pipe only stays busy if nothing else sits in that chain.  Everything that is not a layer
+// therefore runs in the SHADOW of an MMA wait, one tile ahead or behind:
+//   * the input assembly of the NEXT tile (stages A1-A4: staged record / G-buffer texel -> x, local wi/wo) runs
+//     after one of this tile's layers has been issued and leaves its result in registers;
+//   * the output of the PREVIOUS tile (stage B7 softplus, C2 accumulate, C3 store) runs after this tile's layer 1
+//     has been issued; in the light loop the accumulate of light l runs after layer 4 of light l+1 has been issued
+//     and the geometry of light l+1 (stage C1) after layer 5 of light l.
 template <int L, int H, bool kBf16, int NWG, bool kShade>
-__global__ void __launch_bounds__(NWG * 128, 1)
+__global__ void __launch_bounds__(Tc<L, H, kBf16, NWG, kShade>::kThreads, 1)
 tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restrict__ frames, int64_t n,
           FrameParams fr, LightParams lights, float* __restrict__ out)
 {
@@ -314,26 +361,30 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const uint32_t s_wimg = base;
     const uint32_t s_lat = s_wimg + kWimgPad;
     const uint32_t s_stage = s_lat + T::kLatBytes;
-    const uint32_t s_bars = s_stage + NWG * T::kStageBytes;
-    const uint32_t s_tmem = s_bars + NWG * 16u;
+    const uint32_t s_bars = s_stage + NWG * T::kStages * T::kStageBytes;
+    const uint32_t s_tmem = s_bars + NWG * 32u;
     uint8_t* g_wimg = gbase;
     uint8_t* g_lat = g_wimg + kWimgPad;
     uint8_t* g_stage = g_lat + T::kLatBytes;
-    uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStageBytes + NWG * 16u);
+    uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStages * T::kStageBytes + NWG * 32u);
 
     const int tid = threadIdx.x;
+#ifdef NBSDF_CLOCK_PROBE
+    if (blockIdx.x == 0 && tid == 0) { g_clock_probe[0] = (unsigned long long)clock64(); g_clock_probe[1] = global_timer_ns(); }
+#endif
     const int t = tid & 127;               // row within the tile == TMEM lane
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // warp-uniform for the compiler
-    const int wg = warp >> 2;
-    const bool issuer = (warp & 3) == 0;   // warp 0 of each warpgroup issues its MMAs and bulk copies (one elected lane)
+    // warps [0, 4 NWG): the warpgroups that own tile rows; warp 4 NWG + i: the MMA / bulk-copy issuer of warpgroup i
+    const bool issuer = warp >= NWG * 4;
+    const int wg = issuer ? warp - NWG * 4 : warp >> 2;          // >= NWG: padding warp, idle
     constexpr TcLayout lay = T::kLay;
 
     // ---- prologue: weights image + packed latents -> shared memory, barriers, TMEM ----
     // The weight image is immutable after nbsdf_create, so it is fetched before the grid-dependency wait and overlaps
     // the tail of the previous kernel on the stream; everything a previous kernel or copy may write comes after it.
     pdl_launch_dependents();
-    const uint32_t mma_bar = s_bars + (uint32_t)wg * 16u;
-    const uint32_t q_bar = mma_bar + 8u;
+    const uint32_t mma_bar = s_bars + (uint32_t)wg * 32u;
+    const uint32_t q_bar = mma_bar + 8u;            // two of them: one per staging buffer
     const uint32_t w_bar = s_tmem + 8u;
     if (warp == 0 && elect_one()) {
         mbar_init(w_bar, 1);
@@ -347,9 +398,10 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         }
     }
     __syncwarp();
-    if (issuer && elect_one()) {
+    if (issuer && wg < NWG && elect_one()) {
         mbar_init(mma_bar, 1);
         mbar_init(q_bar, 1);
+        mbar_init(q_bar + 8u, 1);
         fence_mbar_init();
     }
     __syncwarp();
@@ -378,7 +430,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     // bias constants (c0, c1, c2) as packed pairs; the CTA-wide constant block is written once per kernel by warpgroup 0
     const uint32_t c01 = pack2<kBf16, false>(tc_bias_const(kBf16, 0), tc_bias_const(kBf16, 1));
     const uint32_t c2z = pack2<kBf16, false>(tc_bias_const(kBf16, 2), 0.0f);
-    if (wg == 0) {
+    if (!issuer && wg == 0) {
         uint32_t ones[8] = { c01, c2z, 0u, 0u, 0u, 0u, 0u, 0u };
         tmem_st8(tmem_base + lane_off + T::kOneCol, ones);
         tmem_wait_st();
@@ -394,23 +446,28 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const int64_t n_tiles = (n_items + 127) / 128;
     const int64_t stride = (int64_t)gridDim.x * NWG;
     const int64_t first = (int64_t)blockIdx.x * NWG + wg;
-    uint32_t mma_phase = 0, q_phase = 0;
-    bool weights_ready = false;
-    const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStageBytes;
-    const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStageBytes;
+    uint32_t mma_phase = 0;
+    const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStages * T::kStageBytes;
+    const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStages * T::kStageBytes;
 
+    // eval: full tiles are staged in shared memory by bulk copies, two buffers per warpgroup; the tile processed in
+    // iteration k of this warpgroup lives in buffer k & 1 and completes phase (k >> 1) & 1 of that buffer's mbarrier.
     auto tile_is_bulk = [&](int64_t tile) { return !kShade && tile < n_tiles && (tile + 1) * 128 <= n_items; };
-    if (issuer && tile_is_bulk(first) && elect_one()) {
-        mbar_expect_tx(q_bar, T::kStageBytes);
-        bulk_g2s(my_stage, q + first * 128, T::kStageBytes, q_bar);
-    }
-    __syncwarp();
+    auto stage_request = [&](int64_t tile, uint32_t k) {      // one elected lane
+        if (tile_is_bulk(tile)) {
+            mbar_expect_tx(q_bar + 8u * (k & 1u), T::kStageBytes);
+            bulk_g2s(my_stage + (k & 1u) * T::kStageBytes, q + tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
+        }
+    };
 
-    // One MMA round: publish the A operand this thread just wrote, let the issuer lane issue, wait for completion.
+    // Hand-over between a warpgroup and its issuer warp, one named barrier (128 arrivals + the 32 waiting issuer lanes):
+    // the owning threads never block here.  The MMA that follows is issued only after every owning thread has arrived,
+    // which orders both the operand it reads (tcgen05.st ... wait::st) and the accumulator it overwrites
+    // (tcgen05.ld ... wait::ld) of all 128 rows before it.
     auto publish = [&]() {
         tmem_wait_st();
         tc_fence_before();
-        named_bar_sync(1 + wg, 128);
+        named_bar_arrive(1 + wg, 160);
     };
     auto await_mma = [&]() {
         mbar_wait(mma_bar, mma_phase);
@@ -418,8 +475,74 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         tc_fence_after();
     };
 
-    // shade: this thread's G-buffer texel of the NEXT tile is requested one tile ahead and lands in registers while the
-    // current tile computes (52 B/pixel, perfectly coalesced float4 planes)
+    if (issuer) {
+        // =========================== MMA / bulk-copy issuer warp of warpgroup wg ===========================
+        setmaxnreg_dec<T::kIssuerRegs>();
+        // Mirrors the owning warpgroup's static layer sequence: wait for "operand ready", issue the layer, commit.
+        // Blocking in tcgen05.mma issue (the tensor pipe's queue is shallow) costs nothing here.
+        auto ready = [&]() {
+            named_bar_sync(1 + wg, 160);
+            tc_fence_after();
+        };
+        if (!kShade && wg < NWG && elect_one()) {
+            stage_request(first, 0u);
+            stage_request(first + stride, 1u);
+        }
+        __syncwarp();
+        uint32_t k = 0;
+        for (int64_t tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
+            ready();
+            if (elect_one()) {
+                if (k == 0) {
+                    stage_request(first + 2 * stride, 2u);    // buffer 0 has been read by every thread of the warpgroup
+                    mbar_wait(w_bar, 0);
+                }
+                issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
+            }
+            __syncwarp();
+            ready();
+            if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[1], mma_bar);
+            __syncwarp();
+            if constexpr (T::kMerged) {
+                ready();
+                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, col0 + T::kTailCol, w_s[2], mma_bar);
+                __syncwarp();
+                ready();                                      // follows assemble(next): staging buffer (k + 1) & 1 is free
+                if (elect_one()) {
+                    stage_request(tile + 3 * stride, k + 3u);
+                    issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[3], mma_bar);
+                }
+                __syncwarp();
+                ready();
+                if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                __syncwarp();
+            } else {
+                ready();
+                if (elect_one()) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
+                __syncwarp();
+                const int n_rounds = kShade ? lights.n : 1;
+                for (int l = 0; l < n_rounds; ++l) {
+                    ready();
+                    if (elect_one()) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
+                    __syncwarp();
+                    ready();                                  // eval: follows assemble(next)
+                    if (elect_one()) {
+                        if (!kShade) stage_request(tile + 3 * stride, k + 3u);
+                        issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                    }
+                    __syncwarp();
+                    ready();
+                    if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[5], mma_bar);
+                    __syncwarp();
+                }
+            }
+        }
+    } else {
+    // =========================== warpgroup wg: owns rows, runs A1-A4, epilogues, B7, C1-C3 ===========================
+    if constexpr (T::kOwnerRegs > T::kBaseRegs) setmaxnreg_inc<T::kOwnerRegs>();
+
+    // shade: this thread's G-buffer texel is requested one tile before it is assembled and lands in registers
+    // (52 B/pixel, perfectly coalesced float4 planes)
     float4 pf_pos = make_float4(0.f, 0.f, 0.f, 1.f), pf_nu = make_float4(0.f, 0.f, 1.f, 0.f), pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
     int pf_mat = -1;
     auto gbuf_request = [&](int64_t tile) {
@@ -431,205 +554,250 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             pf_mat = __ldg(fr.material + it);
         }
     };
-    if (kShade) gbuf_request(first);
+    // ---- per-thread state of the tile that starts next (written by assemble(), one tile ahead) ----
+    uint32_t x[T::K1p / 2];             // layer-1 operand [z, u', v', lf, c0, c1, c2, 0...] as packed pairs (eval: held in
+                                        // registers until the tile starts; shade: stored to TMEM by assemble())
+    uint32_t ytail[3];                  // eval: packed [wi, wo]; shade: the same for the light whose MLP-B starts next
+    int material = -1;
+    float px = 0.0f, py = 0.0f, pz = 0.0f, wo_l[3] = { 0.0f, 0.0f, 1.0f };      // shade: world position, local view direction
+    Frame f;                                                                     // shade: local shading frame
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { f.t[c] = c == 0; f.b[c] = c == 1; f.n[c] = c == 2; }
 
-    for (int64_t tile = first; tile < n_tiles; tile += stride) {
-        const int64_t item = tile * 128 + t;
-        const bool live = item < n_items;
-
-        // ---- stages A1-A4: fetch + assemble ----
-        Assembled a;
-        a.up = a.vp = 0.0f; a.lf = 0.0f; a.material = -1;
-        a.wi[0] = a.wi[1] = 0.0f; a.wi[2] = 1.0f; a.wo[0] = a.wo[1] = 0.0f; a.wo[2] = 1.0f;
-        float px = 0.0f, py = 0.0f, pz = 0.0f;
-        Frame f;
-        if (!kShade) {
+    // stages A1-A4 for `tile` (iteration k of this warpgroup): fetch + assemble into the state above
+    auto assemble = [&](int64_t tile, uint32_t k) {
+        const int64_t it = tile * 128 + t;
+        float up, vp, lf;
+        if constexpr (!kShade) {
             nbsdf_query rec;
             rec.u = rec.v = 0.0f; rec.footprint = 1.0f; rec.material = -1;
             rec.wi[0] = rec.wi[1] = 0.0f; rec.wi[2] = 1.0f; rec.wo[0] = rec.wo[1] = 0.0f; rec.wo[2] = 1.0f;
-            if (tile_is_bulk(tile)) {
-                mbar_wait(q_bar, q_phase);
-                q_phase ^= 1u;
-                const uint2* r2 = reinterpret_cast<const uint2*>(my_stage_g + t * sizeof(nbsdf_query));
-                uint2 w0 = r2[0], w1 = r2[1], w2 = r2[2], w3 = r2[3], w4 = r2[4];
+            const bool bulk = tile_is_bulk(tile);
+            const bool direct = !bulk && tile < n_tiles && it < n_items;
+            auto unpack = [&](const uint2 w0, const uint2 w1, const uint2 w2, const uint2 w3, const uint2 w4) {
                 rec.u = __uint_as_float(w0.x); rec.v = __uint_as_float(w0.y);
                 rec.footprint = __uint_as_float(w1.x); rec.material = (int)w1.y;
                 rec.wi[0] = __uint_as_float(w2.x); rec.wi[1] = __uint_as_float(w2.y); rec.wi[2] = __uint_as_float(w3.x);
                 rec.wo[0] = __uint_as_float(w3.y); rec.wo[1] = __uint_as_float(w4.x); rec.wo[2] = __uint_as_float(w4.y);
-            } else if (live) {
-                const uint2* r2 = reinterpret_cast<const uint2*>(q + item);
-                uint2 w0 = __ldg(r2), w1 = __ldg(r2 + 1), w2 = __ldg(r2 + 2), w3 = __ldg(r2 + 3), w4 = __ldg(r2 + 4);
-                rec.u = __uint_as_float(w0.x); rec.v = __uint_as_float(w0.y);
-                rec.footprint = __uint_as_float(w1.x); rec.material = (int)w1.y;
-                rec.wi[0] = __uint_as_float(w2.x); rec.wi[1] = __uint_as_float(w2.y); rec.wi[2] = __uint_as_float(w3.x);
-                rec.wo[0] = __uint_as_float(w3.y); rec.wo[1] = __uint_as_float(w4.x); rec.wo[2] = __uint_as_float(w4.y);
+            };
+            if (bulk) {
+                mbar_wait(q_bar + 8u * (k & 1u), (k >> 1) & 1u);
+                const uint2* r2 = reinterpret_cast<const uint2*>(my_stage_g + (k & 1u) * T::kStageBytes + t * sizeof(nbsdf_query));
+                unpack(r2[0], r2[1], r2[2], r2[3], r2[4]);
+            } else if (direct) {
+                const uint2* r2 = reinterpret_cast<const uint2*>(q + it);
+                unpack(__ldg(r2), __ldg(r2 + 1), __ldg(r2 + 2), __ldg(r2 + 3), __ldg(r2 + 4));
             }
-            a.up = wrap01(rec.u); a.vp = wrap01(rec.v); a.lf = log_footprint<true>(rec.footprint);
-            a.material = rec.material;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { a.wi[c] = rec.wi[c]; a.wo[c] = rec.wo[c]; }
-            if (frames != nullptr && live) {
-                const float2* fp2 = reinterpret_cast<const float2*>(frames + 6 * item);
+            up = wrap01(rec.u); vp = wrap01(rec.v); lf = log_footprint<true>(rec.footprint);
+            material = rec.material;
+            float wi[3] = { rec.wi[0], rec.wi[1], rec.wi[2] }, wo[3] = { rec.wo[0], rec.wo[1], rec.wo[2] };
+            if (frames != nullptr && (bulk || direct)) {
+                const float2* fp2 = reinterpret_cast<const float2*>(frames + 6 * it);
                 const float2 f0 = __ldg(fp2), f1 = __ldg(fp2 + 1), f2 = __ldg(fp2 + 2);
-                f = make_frame(f0.x, f0.y, f1.x, f1.y, f2.x, f2.y);
-                to_local(f, rec.wi[0], rec.wi[1], rec.wi[2], a.wi);
-                to_local(f, rec.wo[0], rec.wo[1], rec.wo[2], a.wo);
+                const Frame ff = make_frame(f0.x, f0.y, f1.x, f1.y, f2.x, f2.y);
+                to_local(ff, rec.wi[0], rec.wi[1], rec.wi[2], wi);
+                to_local(ff, rec.wo[0], rec.wo[1], rec.wo[2], wo);
             }
+            ytail[0] = pack2<kBf16, false>(wi[0], wi[1]);
+            ytail[1] = pack2<kBf16, false>(wi[2], wo[0]);
+            ytail[2] = pack2<kBf16, false>(wo[1], wo[2]);
         } else {
             const float4 pos = pf_pos, nu = pf_nu, tv = pf_tv;
-            a.material = pf_mat;
+            material = pf_mat;
             gbuf_request(tile + stride);
             px = pos.x; py = pos.y; pz = pos.z;
             f = make_frame(nu.x, nu.y, nu.z, tv.x, tv.y, tv.z);
-            float vx = fr.cam[0] - px, vy = fr.cam[1] - py, vz = fr.cam[2] - pz;
+            const float vx = fr.cam[0] - px, vy = fr.cam[1] - py, vz = fr.cam[2] - pz;
             const float inv = rsqrtf(vx * vx + vy * vy + vz * vz);
-            to_local(f, vx * inv, vy * inv, vz * inv, a.wo);
-            a.up = wrap01(nu.w); a.vp = wrap01(tv.w); a.lf = log_footprint<true>(pos.w);
+            to_local(f, vx * inv, vy * inv, vz * inv, wo_l);
+            up = wrap01(nu.w); vp = wrap01(tv.w); lf = log_footprint<true>(pos.w);
         }
-
-        // ---- layer-1 operand x = [z, u', v', lf, 0...] -> AY ----
-        {
-            const int m = a.material < 0 ? 0 : a.material;
-            uint32_t x[T::K1p / 2];
-            const uint4* zrow = reinterpret_cast<const uint4*>(g_lat + (size_t)m * L * 2);
+        const int m = material < 0 ? 0 : material;
+        const uint4* zrow = reinterpret_cast<const uint4*>(g_lat + (size_t)m * L * 2);
 #pragma unroll
-            for (int i = 0; i < L / 8; ++i) {
-                const uint4 z4 = zrow[i];
-                x[4 * i] = z4.x; x[4 * i + 1] = z4.y; x[4 * i + 2] = z4.z; x[4 * i + 3] = z4.w;
-            }
-            x[L / 2] = pack2<kBf16, false>(a.up, a.vp);
-            x[L / 2 + 1] = pack2<kBf16, false>(a.lf, tc_bias_const(kBf16, 0));
-            x[L / 2 + 2] = pack2<kBf16, false>(tc_bias_const(kBf16, 1), tc_bias_const(kBf16, 2));
+        for (int i = 0; i < L / 8; ++i) {
+            const uint4 z4 = zrow[i];
+            x[4 * i] = z4.x; x[4 * i + 1] = z4.y; x[4 * i + 2] = z4.z; x[4 * i + 3] = z4.w;
+        }
+        x[L / 2] = pack2<kBf16, false>(up, vp);
+        x[L / 2 + 1] = pack2<kBf16, false>(lf, tc_bias_const(kBf16, 0));
+        x[L / 2 + 2] = pack2<kBf16, false>(tc_bias_const(kBf16, 1), tc_bias_const(kBf16, 2));
 #pragma unroll
-            for (int i = L / 2 + 3; i < T::K1p / 2; ++i) x[i] = 0u;
+        for (int i = L / 2 + 3; i < T::K1p / 2; ++i) x[i] = 0u;
+        if constexpr (kShade) {         // AY is a region of its own and dead by now (the last layer 4 has completed)
 #pragma unroll
             for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
-            if constexpr (T::kMerged) {   // tail block of the merged layer: [wi, wo, c0, c1, c2, 0...]
-                uint32_t y[8];
-                y[0] = pack2<kBf16, false>(a.wi[0], a.wi[1]);
-                y[1] = pack2<kBf16, false>(a.wi[2], a.wo[0]);
-                y[2] = pack2<kBf16, false>(a.wo[1], a.wo[2]);
-                y[3] = c01;
-                y[4] = c2z;
+        }
+    };
+
+    // shade, stage C1: geometry of light l at this pixel -> packed [wi_local, wo_local] and E * cos
+    float w_cur[3] = { 0.0f, 0.0f, 0.0f }, w_nxt[3] = { 0.0f, 0.0f, 0.0f };
+    auto light_tail = [&](int l) {
+        float wiw[3], E[3], wi[3];
+        light_sample(lights.light[l], px, py, pz, wiw, E);
+        to_local(f, wiw[0], wiw[1], wiw[2], wi);
+        const float cs = fmaxf(wi[2], 0.0f);
+        ytail[0] = pack2<kBf16, false>(wi[0], wi[1]);
+        ytail[1] = pack2<kBf16, false>(wi[2], wo_l[0]);
+        ytail[2] = pack2<kBf16, false>(wo_l[1], wo_l[2]);
 #pragma unroll
-                for (int i = 5; i < 8; ++i) y[i] = 0u;
-                tmem_st8(lane_taddr + T::kTailCol, y);
-            }
-        }
+        for (int c = 0; c < 3; ++c) w_nxt[c] = E[c] * cs;
+    };
+    // [wi, wo, c0, c1, c2, 0...] -> 8 A-operand columns
+    auto store_tail = [&](uint32_t taddr) {
+        uint32_t y[8] = { ytail[0], ytail[1], ytail[2], c01, c2z, 0u, 0u, 0u };
+        tmem_st8(taddr, y);
+    };
 
-        // ---- MLP-A (B1-B3) ----
-        publish();                            // every thread has consumed its staged record and stored x
-        if (issuer) {
-            if (elect_one()) {
-                const int64_t next = tile + stride;
-                if (tile_is_bulk(next)) {          // stream the next tile's records in while this one computes
-                    mbar_expect_tx(q_bar, T::kStageBytes);
-                    bulk_g2s(my_stage, q + next * 128, T::kStageBytes, q_bar);
-                }
-                if (!weights_ready) mbar_wait(w_bar, 0);
-                issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
-            }
-            weights_ready = true;
-            __syncwarp();
-        }
-        await_mma();
-
-        epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-        publish();
-        if (issuer) {
-            if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[1], mma_bar);
-            __syncwarp();
-        }
-        await_mma();
-        epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-        float rad[3] = { 0.0f, 0.0f, 0.0f };
-        // last two layers of MLP-B + softplus (B5-B7); g1 has just been published as the A operand
-        auto finish_mlp_b = [&](uint32_t w5, uint32_t w6, const float E[3], float cs) {
-            if (issuer) {
-                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w5, mma_bar);
-                __syncwarp();
-            }
-            await_mma();
-            epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-            publish();
-            if (issuer) {
-                if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w6, mma_bar);
-                __syncwarp();
-            }
-            await_mma();
-            uint32_t o[4];
-            tmem_ld4(acc_t, o);
-            tmem_wait_ld();
+    // deferred output of the tile finished last: raw output-layer values, their item and what to do with them
+    float o_prev[3] = { 0.0f, 0.0f, 0.0f }, rad[3] = { 0.0f, 0.0f, 0.0f };
+    int64_t prev_item = 0;
+    int prev_kind = 0;                  // 0: nothing pending / dead row, 1: store, 2: background (store zeros)
+    auto flush_output = [&]() {
+        if (prev_kind != 0) {
+            float r[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float v = softplus<true>(__uint_as_float(o[c]));
-                rad[c] = kShade ? fmaf(v * E[c], cs, rad[c]) : v;
+                const float v = softplus<true>(o_prev[c]);
+                r[c] = kShade ? fmaf(v, w_cur[c], rad[c]) : v;
+                if (prev_kind == 2) r[c] = 0.0f;
             }
-        };
+            out[3 * prev_item + 0] = r[0];
+            out[3 * prev_item + 1] = r[1];
+            out[3 * prev_item + 2] = r[2];
+        }
+        prev_kind = 0;
+        rad[0] = rad[1] = rad[2] = 0.0f;
+    };
+    auto load_output = [&]() {
+        uint32_t o[4];
+        tmem_ld4(acc_t, o);
+        tmem_wait_ld();
+#pragma unroll
+        for (int c = 0; c < 3; ++c) o_prev[c] = __uint_as_float(o[c]);
+    };
+
+    if (kShade) gbuf_request(first);
+    if (first < n_tiles) assemble(first, 0u);
+
+#ifdef NBSDF_PHASE_PROBE
+    long long ph_acc[24], ph_last = clock64();
+#pragma unroll
+    for (int i = 0; i < 24; ++i) ph_acc[i] = 0;
+#endif
+    uint32_t k = 0;
+    for (int64_t tile = first; tile < n_tiles; tile += stride, ++k) {
+        const int64_t item = tile * 128 + t;
+        const int kind = item < n_items ? (material < 0 ? 2 : 1) : 0;
+
+        // ---- layer-1 operand (and the merged layer's tail block) -> TMEM ----
+        if constexpr (!kShade) {
+#pragma unroll
+            for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
+        }
+        if constexpr (T::kMerged) store_tail(lane_taddr + T::kTailCol);
+        NBSDF_PHASE(0);
+
+        // ---- MLP-A (B1-B3) ----
+        publish();                                        // -> layer 1 (short: nothing is put in its shadow)
+        NBSDF_PHASE(1);
+        NBSDF_PHASE(2);
+        await_mma();
+        NBSDF_PHASE(3);
+        epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+        NBSDF_PHASE(4);
+        publish();                                        // -> layer 2
+        flush_output();                                   // shadow of layer 2: the previous tile's B7 / C2-C3
+        NBSDF_PHASE(5);
+        if constexpr (kShade) light_tail(0);              //                    and C1 of the first light
+        await_mma();
+        NBSDF_PHASE(6);
+        epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+        NBSDF_PHASE(7);
+
         if constexpr (T::kMerged) {
             // ---- merged layers 3+4 (B3-B4): (W4f W3) h2 + W4a [wi, wo] + (W4f b3 + b4); K = H from AH + tail block ----
-            publish();
-            if (issuer) {
-                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, col0 + T::kTailCol, w_s[2], mma_bar);
-                __syncwarp();
-            }
+            publish();                                    // -> merged layer
+            NBSDF_PHASE(8);
+            assemble(tile + stride, k + 1u);              // shadow of the merged layer: A1-A4 of the next tile
+            NBSDF_PHASE(12);
             await_mma();
-            epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-            publish();
-            const float E1[3] = { 1.0f, 1.0f, 1.0f };
-            finish_mlp_b(w_s[3], w_s[4], E1, 1.0f);
+            NBSDF_PHASE(9);
+            epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+            NBSDF_PHASE(10);
+            publish();                                    // -> layer 5; the issuer also refills the staging buffer just read
+            NBSDF_PHASE(11);
+            await_mma();
+            NBSDF_PHASE(13);
+            epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+            NBSDF_PHASE(14);
+            publish();                                    // -> layer 6
+            NBSDF_PHASE(15);
+            await_mma();
+            NBSDF_PHASE(16);
+            load_output();
+            NBSDF_PHASE(17);
         } else {
-            publish();
-            if (issuer) {
-                if (elect_one()) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
-                __syncwarp();
-            }
+            publish();                                    // -> layer 3
             await_mma();
             epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t);      // feat (linear) -> AY columns [0, 16)
+            store_tail(ay_t + 16);                                // [wi, wo, c] of the query / of light 0
+#pragma unroll
+            for (int c = 0; c < 3; ++c) w_cur[c] = kShade ? w_nxt[c] : 1.0f;
 
             // ---- MLP-B (B4-B7), once per query / once per light (C1-C3) ----
             const int n_rounds = kShade ? lights.n : 1;
             for (int l = 0; l < n_rounds; ++l) {
-                float E[3] = { 1.0f, 1.0f, 1.0f };
-                float cs = 1.0f;
-                if (kShade) {
-                    float wiw[3];
-                    light_sample(lights.light[l], px, py, pz, wiw, E);
-                    to_local(f, wiw[0], wiw[1], wiw[2], a.wi);
-                    cs = fmaxf(a.wi[2], 0.0f);
-                }
-                uint32_t y[8];
-                y[0] = pack2<kBf16, false>(a.wi[0], a.wi[1]);
-                y[1] = pack2<kBf16, false>(a.wi[2], a.wo[0]);
-                y[2] = pack2<kBf16, false>(a.wo[1], a.wo[2]);
-                y[3] = c01;
-                y[4] = c2z;
+                publish();                                // -> layer 4 (also: this thread has read the previous light's output)
+                if constexpr (kShade) {                   // shadow of layer 4: C2 of the previous light
+                    if (l > 0) {
 #pragma unroll
-                for (int i = 5; i < 8; ++i) y[i] = 0u;
-                tmem_st8(ay_t + 16, y);
-                publish();
-                if (issuer) {
-                    if (elect_one()) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
-                    __syncwarp();
+                        for (int c = 0; c < 3; ++c) {
+                            rad[c] = fmaf(softplus<true>(o_prev[c]), w_cur[c], rad[c]);
+                            w_cur[c] = w_nxt[c];
+                        }
+                    }
+                } else {
+                    assemble(tile + stride, k + 1u);      // shadow of layer 4: A1-A4 of the next tile
                 }
                 await_mma();
-                epilogue_to_a<H, true, kBf16>(acc_t, ah_t);
-                publish();
-                finish_mlp_b(w_s[4], w_s[5], E, cs);
+                epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+                publish();                                // -> layer 5; eval: the issuer also refills the staging buffer just read
+                if constexpr (kShade) {                   // shadow of layer 5: C1 of the next light, or A1-A4 of the next tile
+                    if (l + 1 < n_rounds) {
+                        light_tail(l + 1);
+                        store_tail(ay_t + 16);            // layer 4 of light l has completed: its operand may be replaced
+                    } else {
+                        assemble(tile + stride, k + 1u);
+                    }
+                }
+                await_mma();
+                epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+                publish();                                // -> layer 6
+                await_mma();
+                load_output();
             }
         }
-        if (live) {
-            const bool bg = a.material < 0;
-            out[3 * item + 0] = bg ? 0.0f : rad[0];
-            out[3 * item + 1] = bg ? 0.0f : rad[1];
-            out[3 * item + 2] = bg ? 0.0f : rad[2];
-        }
+        prev_item = item;
+        prev_kind = kind;
     }
+    flush_output();
+#ifdef NBSDF_PHASE_PROBE
+    if (blockIdx.x == 0 && tid == 0) {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) g_phase_probe[i] = ph_acc[i];
+        g_phase_probe[24] = (long long)k;
+    }
+#endif
+    }   // role
 
     // ---- teardown ----
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem_base, 512);
+#ifdef NBSDF_CLOCK_PROBE
+    if (blockIdx.x == 0 && tid == 0) { g_clock_probe[2] = (unsigned long long)clock64(); g_clock_probe[3] = global_timer_ns(); }
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -637,7 +805,7 @@ template <int L, int H, bool kBf16, bool kShade>
 static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_query* q, const float* frames, int64_t n,
                               const FrameParams& fr, const LightParams& lights, float* out, cudaStream_t s, bool init_only)
 {
-    constexpr int NWG = H == 128 ? 2 : (H == 32 ? (kShade ? 6 : NBSDF_NWG32_EVAL) : (kShade ? 4 : NBSDF_NWG64_EVAL));
+    constexpr int NWG = H == 128 ? 2 : (H == 32 ? (kShade ? 5 : NBSDF_NWG32_EVAL) : (kShade ? 4 : NBSDF_NWG64_EVAL));
     using T = Tc<L, H, kBf16, NWG, kShade>;
     auto kern = tc_kernel<L, H, kBf16, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());
@@ -648,7 +816,7 @@ static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_que
     if (grid < 1) grid = 1;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(NWG * 128);
+    cfg.blockDim = dim3(T::kThreads);
     cfg.dynamicSmemBytes = T::smem_bytes();
     cfg.stream = s;
     cudaLaunchAttribute attr[1];
@@ -702,7 +870,22 @@ cudaError_t launch_eval_tc(const NetParams& net, int precision, int num_sms, con
 cudaError_t launch_shade_tc(const NetParams& net, int precision, int num_sms, const FrameParams& fr,
                             const LightParams& lights, float* out, cudaStream_t s)
 {
+    // no light: the radiance is exactly zero and the kernel's light loop may assume at least one round
+    if (lights.n == 0) return cudaMemsetAsync(out, 0, (size_t)fr.n_pixels * 3 * sizeof(float), s);
     return dispatch<true>(net, precision, num_sms, nullptr, nullptr, 0, fr, lights, out, s, false);
 }
 
 }  // namespace nbsdf
+
+#ifdef NBSDF_PHASE_PROBE
+extern "C" int nbsdf_debug_phase_probe(long long* out32)
+{
+    return (int)cudaMemcpyFromSymbol(out32, nbsdf::g_phase_probe, 32 * sizeof(long long));
+}
+#endif
+#ifdef NBSDF_CLOCK_PROBE
+extern "C" int nbsdf_debug_clock_probe(unsigned long long* out4)
+{
+    return (int)cudaMemcpyFromSymbol(out4, nbsdf::g_clock_probe, 4 * sizeof(unsigned long long));
+}
+#endif

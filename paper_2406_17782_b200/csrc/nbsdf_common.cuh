@@ -167,7 +167,10 @@ __host__ __device__ constexpr int pad16(int k) { return (k + 15) & ~15; }
 //                  Multiply-adds: H (H + 6) merged vs 2 F H + 6 H separate -- equal at H = 64 (F = 32), fewer at H = 32,
 //                  twice as many at H = 128 (which is why H = 128 keeps six layers).  Its last K step reads
 //                  [wi, wo, c0, c1, c2] from a per-warpgroup tail block instead of the CTA-wide bias-constant block.
-__host__ __device__ constexpr bool tc_eval_merged(int H) { return H <= 64; }
+#ifndef NBSDF_EVAL_MERGE_MAX_H
+#define NBSDF_EVAL_MERGE_MAX_H 64
+#endif
+__host__ __device__ constexpr bool tc_eval_merged(int H) { return H <= NBSDF_EVAL_MERGE_MAX_H; }
 
 __host__ __device__ constexpr TcLayout tc_layout(int L, int H, bool merged)
 {

@@ -256,6 +256,7 @@ struct Tc {
     static constexpr int kOwnerRegsRaw = kBaseRegs + kIssuerWarps * 32 * (kBaseRegs - kIssuerRegs) / (NWG * 128) / 8 * 8;
     static constexpr int kOwnerRegs = kOwnerRegsRaw > 248 ? 248 : kOwnerRegsRaw;
     static_assert(kThreads <= 1024, "CTA size");
+    static constexpr bool kTwoLoads = kOwnerRegs >= (kShade ? 160 : 100);         // epilogue register budget (see epilogue_to_a)
     // TMEM columns of one warpgroup.  eval: x, the hidden activations and y share ONE A-operand region (each is dead
     // before the next is written); shade: y = [feat, wi, wo] must survive the light loop, so it gets its own region.
     // Merged eval adds an 8-column tail block [wi, wo, c0, c1, c2, 0...]: the last K step of the merged layer.
@@ -273,7 +274,6 @@ struct Tc {
     static constexpr uint32_t kLatBytes = 64 * 32 * 2;            // packed latent table, max M x max L
     static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);
     static constexpr uint32_t kStages = 2;                        // staging buffers per warpgroup
-    static constexpr bool kTwoLoads = NWG * 128 * 160 <= 65536 || !kShade;   // epilogue register budget (see epilogue_to_a)
 
     __host__ __device__ static constexpr uint32_t wimg_bytes() { return kLay.total; }
     __host__ __device__ static constexpr uint32_t smem_bytes()

@@ -7,6 +7,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "nbsdf_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "nbsdf_oracle_paper.c")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 # wire format of the inputs (query = position, size, wi, wo + material latent id)
@@ -24,9 +25,9 @@ class _Dims(C.Structure):
 
 def build(force=False):
     """Compile the oracle with gcc (no fast-math, no contraction).  Building is not using."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-                               "-o", _LIB, _SRC, "-lm"])
+                               "-o", _LIB] + _SRCS + ["-lm"])
     return _LIB
 
 
@@ -59,6 +60,18 @@ def _load():
         lib.oracle_shade_frame.argtypes = [C.c_void_p] * 8 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
                                                               C.c_int, C.c_void_p, C.c_int]
         lib.oracle_max_threads.restype = C.c_int
+        for name in ("oracle_leaky", "oracle_size01"):
+            getattr(lib, name).restype = C.c_double
+            getattr(lib, name).argtypes = [C.c_double]
+        lib.oracle_inv_logmap.restype = C.c_double
+        lib.oracle_inv_logmap.argtypes = [C.c_double, C.c_double]
+        lib.oracle_oneblob.restype = None
+        lib.oracle_oneblob.argtypes = [C.c_double, C.c_int, C.c_void_p]
+        lib.oracle_pd_eval.restype = C.c_int
+        lib.oracle_pd_eval.argtypes = [C.c_void_p] * 7 + [C.c_int64, C.c_void_p, C.c_void_p, C.c_int]
+        lib.oracle_pd_shade_frame.restype = C.c_int
+        lib.oracle_pd_shade_frame.argtypes = [C.c_void_p] * 9 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                                                 C.c_int, C.c_void_p, C.c_int]
         global _all_threads
         _all_threads = int(lib.oracle_max_threads())      # before any call narrows the OpenMP team
         _lib = lib
@@ -153,3 +166,86 @@ def to_local(n, t, w):
 def max_threads():
     _load()
     return _all_threads
+
+
+# ---------------------------------------------------------------------------------------------------
+# paper-structured decoder (nbsdf_oracle_paper.c)
+def _pack_pd(weights, biases, latents, albedos):
+    """weights/biases: 7 arrays (fusion 2 + angular decoder 5), W_k row-major [out][in]; latents [M][L];
+    albedos [M][12] = kd_warp, kd_weft, ks_warp, ks_weft (RGB each)."""
+    Ws = [_f32(w) for w in weights]
+    bs = [_f32(b).reshape(-1) for b in biases]
+    Z = _f32(latents)
+    A = _f32(albedos)
+    assert len(Ws) == 7 and len(bs) == 7 and Z.ndim == 2
+    M, L = Z.shape
+    assert A.shape == (M, 12)
+    H, F = Ws[0].shape[0], Ws[1].shape[0]
+    shapes = [(H, L + 24), (F, H), (H, F + 5), (H, H), (H, H), (H, H), (4, H)]
+    for w, b, s in zip(Ws, bs, shapes):
+        assert w.shape == s and b.shape == (s[0],), (w.shape, b.shape, s)
+    dims = _Dims(L, H, F, M)
+    Wp = (C.c_void_p * 7)(*[w.ctypes.data for w in Ws])
+    bp = (C.c_void_p * 7)(*[b.ctypes.data for b in bs])
+    return dims, Wp, bp, Z, A, (Ws, bs)
+
+
+def pd_eval_queries(weights, biases, latents, albedos, queries, frames=None, n_threads=0, components=False):
+    """fp64 paper-structured decoder over QUERY_DTYPE records (footprint = size in pattern units; wo.z unused)
+    -> float64 [n][3] (and [n][4] = C_warp, C_weft, S_warp, S_weft when components=True)."""
+    dims, Wp, bp, Z, A, _keep = _pack_pd(weights, biases, latents, albedos)
+    q = np.ascontiguousarray(queries, dtype=QUERY_DTYPE)
+    n = q.shape[0]
+    fr = None
+    if frames is not None:
+        fr = _f32(frames)
+        assert fr.shape == (n, 6)
+    assert n == 0 or int(q["material"].max()) < Z.shape[0], "material id out of range"
+    out = np.empty((n, 3), dtype=np.float64)
+    comp = np.empty((n, 4), dtype=np.float64) if components else None
+    rc = _load().oracle_pd_eval(C.byref(dims), Wp, bp, Z.ctypes.data, A.ctypes.data, q.ctypes.data,
+                                fr.ctypes.data if fr is not None else None, n, out.ctypes.data,
+                                comp.ctypes.data if components else None, _threads(n_threads))
+    assert rc == 0
+    return (out, comp) if components else out
+
+
+def pd_shade_frame(weights, biases, latents, albedos, gbuffer, lights, first=0, count=None, n_threads=0):
+    """fp64 frame shading with the paper-structured decoder (|cos| weighting; pos_fp.w = footprint size)."""
+    dims, Wp, bp, Z, A, _keep = _pack_pd(weights, biases, latents, albedos)
+    pos = _f32(gbuffer["pos_fp"]).reshape(-1, 4)
+    nrm = _f32(gbuffer["nrm_u"]).reshape(-1, 4)
+    tan = _f32(gbuffer["tan_v"]).reshape(-1, 4)
+    mat = np.ascontiguousarray(gbuffer["material"], dtype=np.int32).reshape(-1)
+    npx = mat.shape[0]
+    cam = _f32(gbuffer["cam_pos"]).reshape(3)
+    lt = np.ascontiguousarray(lights, dtype=LIGHT_DTYPE).reshape(-1)
+    if count is None:
+        count = npx - first
+    assert 0 <= first and first + count <= npx
+    assert npx == 0 or int(mat.max()) < Z.shape[0], "material id out of range"
+    out = np.empty((count, 3), dtype=np.float64)
+    rc = _load().oracle_pd_shade_frame(C.byref(dims), Wp, bp, Z.ctypes.data, A.ctypes.data, pos.ctypes.data,
+                                       nrm.ctypes.data, tan.ctypes.data, mat.ctypes.data, first, count,
+                                       cam.ctypes.data, lt.ctypes.data if lt.shape[0] else None, lt.shape[0],
+                                       out.ctypes.data, _threads(n_threads))
+    assert rc == 0
+    return out
+
+
+def oneblob(s, k=8):
+    out = np.empty(k, dtype=np.float64)
+    _load().oracle_oneblob(float(s), int(k), out.ctypes.data)
+    return out
+
+
+def leaky(x):
+    return _load().oracle_leaky(float(x))
+
+
+def size01(x):
+    return _load().oracle_size01(float(x))
+
+
+def inv_logmap(y, k):
+    return _load().oracle_inv_logmap(float(y), float(k))

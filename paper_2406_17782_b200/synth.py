@@ -184,3 +184,82 @@ def config(idx, n=None, width=None, height=None, L=16, H=64, seed=None):
         return {"name": "frame_4k_16lights_edit", "weights": Ws, "biases": bs, "latents": Z, "gbuffer": g,
                 "lights": lights, "edit_material": 3, "edit_latent": z_edit}
     raise ValueError(idx)
+
+
+# ---------------------------------------------------------------------------------------------------
+# Inputs for the paper-structured decoder.  Data only, as above.
+PD_LATENT = 64
+
+
+def pd_layer_shapes(L=PD_LATENT, H=64, F=FEAT_DIM):
+    """fusion (2 layers) + angular decoder (5 layers): [out, in] per layer."""
+    return [(H, L + 24), (F, H), (H, F + 5), (H, H), (H, H), (H, H), (4, H)]
+
+
+def make_pd_network(rng, L=PD_LATENT, H=64, F=FEAT_DIM, bf16_weights=True):
+    """Xavier-uniform weights, biases 0.01*N(0,1).  The output biases are then shifted so that the synthetic network
+    behaves like a BSDF: diffuse components around 1 (positive), log-mapped specular outputs around 3, i.e.
+    S = (e^3 - 1)/100 ~ 0.2 for reflection.  Draw order: W1,b1,...,W7,b7."""
+    Ws, bs = [], []
+    for (n_out, n_in) in pd_layer_shapes(L, H, F):
+        a = math.sqrt(6.0 / (n_in + n_out))
+        W = rng.uniform(-a, a, size=(n_out, n_in)).astype(np.float32)
+        b = (0.01 * rng.standard_normal(n_out)).astype(np.float32)
+        Ws.append(round_to_bf16(W) if bf16_weights else W)
+        bs.append(b)
+    bs[6][0:2] += np.float32(1.0)
+    bs[6][2:4] += np.float32(3.0)
+    return Ws, bs
+
+
+def make_albedos(rng, M):
+    """[M][12] = kd_warp, kd_weft, ks_warp, ks_weft (RGB each) ~ U[0.05, 0.95)."""
+    return rng.uniform(0.05, 0.95, size=(M, 12)).astype(np.float32)
+
+
+def disk_direction(rng, n, transmit_fraction=0.0):
+    """(x, y) uniform in the unit disk (Table 2 samples x, y in (-1,1) and keeps valid pairs),
+    z = +sqrt(1 - x^2 - y^2), negated for a `transmit_fraction` of the samples (BTDF)."""
+    r = np.sqrt(rng.random(n)) * 0.999
+    phi = 2.0 * np.pi * rng.random(n)
+    x, y = r * np.cos(phi), r * np.sin(phi)
+    z = np.sqrt(np.maximum(0.0, 1.0 - x * x - y * y))
+    if transmit_fraction > 0.0:
+        z = np.where(rng.random(n) < transmit_fraction, -z, z)
+    return np.stack([x, y, z], axis=1).astype(np.float32)
+
+
+def make_pd_queries(rng, n, M):
+    """Table 2: position U(0,1)^2, size U(0,1) or U(1,5) with equal probability, directions from
+    the (x, y) disk; a quarter of the incoming directions lie below the surface (transmission).
+    Draw order: u, v, size branch, size, wi, wo, material."""
+    q = np.zeros(n, dtype=QUERY_DTYPE)
+    q["u"] = rng.random(n).astype(np.float32)
+    q["v"] = rng.random(n).astype(np.float32)
+    big = rng.random(n) < 0.5
+    s = rng.random(n)
+    q["footprint"] = np.where(big, 1.0 + 4.0 * s, s).astype(np.float32)
+    q["wi"] = disk_direction(rng, n, 0.25)
+    q["wo"] = disk_direction(rng, n)
+    q["material"] = rng.integers(0, M, n).astype(np.int32) if M > 1 else 0
+    return q
+
+
+def pd_config(kind, n=None, width=None, height=None, H=64, seed=None, M=8):
+    """kind 'eval': batch of Table-2 queries; kind 'frame': the configs[2] G-buffer (footprint size = its uv
+    derivative, in pattern units) with the five direct lights plus one point light BEHIND the fabric."""
+    rng = np.random.default_rng({"eval": 11, "frame": 12}[kind] if seed is None else seed)
+    Ws, bs = make_pd_network(rng, PD_LATENT, H)
+    Z = make_latents(rng, M, PD_LATENT)
+    A = make_albedos(rng, M)
+    out = {"weights": Ws, "biases": bs, "latents": Z, "albedos": A}
+    if kind == "eval":
+        out["queries"] = make_pd_queries(rng, (1 << 20) if n is None else n, M)
+    else:
+        out["gbuffer"] = make_gbuffer(rng, 1920 if width is None else width, 1080 if height is None else height)
+        back = np.zeros(1, dtype=LIGHT_DTYPE)
+        back["type"] = 1
+        back["vec"] = (0.2, -0.1, -0.6)
+        back["rgb"] = (0.3, 0.35, 0.4)
+        out["lights"] = np.concatenate([lights_direct5(), back])
+    return out

@@ -127,6 +127,33 @@ int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float* frames_dev
 int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* gbuf, const nbsdf_light* lights_host, int32_t n_lights,
                       float* radiance_dev, void* cuda_stream);
 
+/* ---- Decoder with the paper's own structure ----
+ * latent 64; one-blob encoding of (u', v', size/5) with 8 bins each, 3 -> 24 channels;
+ * fusion:          W[0]: H x (64+24) leaky ReLU,  W[1]: F x H leaky ReLU                   ("two fully connected layers")
+ * angular decoder: W[2]: H x (F+5) on [feat, wi.xyz, wo.xy],  W[3]: H x H,  W[4]: H x H + skip from W[2]'s output,
+ *                  W[5]: H x H,  W[6]: 4 x H (linear); leaky ReLU (slope 0.01) after all but the last
+ *                  ("five fully connected layers with one skip connection").
+ * Outputs (C_warp, C_weft, g(S_warp), g(S_weft)), g(x) = ln(k x + 1), k = 100 when wi_local.z >= 0 and 1000 below
+ * (PAPER.md:172-177); the library inverts g and combines with the material's albedos (Eq. 8):
+ *   rgb = kd_warp C_warp + kd_weft C_weft + ks_warp S_warp + ks_weft S_weft.
+ * HOST pointers, fp32, row-major [out][in], copied.  Supported: latent_dim 64, hidden 64, feat_dim 32,
+ * precision NBSDF_PREC_FP16 or NBSDF_PREC_BF16 (tensor cores); anything else => NBSDF_E_UNSUPPORTED.
+ * A context made here is used with the same nbsdf_set_latents / nbsdf_eval / nbsdf_shade_frame calls:
+ *   nbsdf_query.footprint and pos_fp.w then hold the footprint SIZE in multiples of the pattern size (clamped to
+ *   [0, 5]), wo.z is ignored, and nbsdf_shade_frame weights each light by |wi_local.z| (transmission contributes). */
+typedef struct {
+    const float* W[7];
+    const float* b[7];
+} nbsdf_paper_weights;
+
+int nbsdf_create_paper(const nbsdf_config* cfg, const nbsdf_paper_weights* weights, nbsdf_ctx** out);
+
+/* Overwrites rows [first, first+count) of the albedo table of a paper-structured context: 12 fp32 per material,
+ * kd_warp, kd_weft, ks_warp, ks_weft (RGB each); the table starts zero-filled.  PAPER.md:198: "to edit albedos ... no
+ * encoder inference is needed".  albedos_host: HOST, copied before return; ordered on cuda_stream like set_latents.
+ * NBSDF_E_INVALID on a context made by nbsdf_create. */
+int nbsdf_set_albedos(nbsdf_ctx* ctx, int32_t first, int32_t count, const float* albedos_host, void* cuda_stream);
+
 /* Frees everything the context owns.  The caller must have synchronised the streams it used.  NULL is allowed. */
 void nbsdf_destroy(nbsdf_ctx* ctx);
 

@@ -15,7 +15,7 @@ NBSDF_PREC_FP32, NBSDF_PREC_BF16, NBSDF_PREC_FP16 = 0, 1, 2
 PRECISIONS = {"fp32": NBSDF_PREC_FP32, "bf16": NBSDF_PREC_BF16, "fp16": NBSDF_PREC_FP16}
 NBSDF_MAX_LIGHTS = 32
 EXPORTS = ["nbsdf_create", "nbsdf_set_latents", "nbsdf_eval", "nbsdf_shade_frame", "nbsdf_destroy",
-           "nbsdf_last_error", "nbsdf_launch_count"]
+           "nbsdf_last_error", "nbsdf_launch_count", "nbsdf_create_paper", "nbsdf_set_albedos"]
 
 
 class NbsdfError(RuntimeError):
@@ -31,6 +31,10 @@ class _Config(C.Structure):
 
 class _Weights(C.Structure):
     _fields_ = [("W", C.c_void_p * 6), ("b", C.c_void_p * 6)]
+
+
+class _PaperWeights(C.Structure):
+    _fields_ = [("W", C.c_void_p * 7), ("b", C.c_void_p * 7)]
 
 
 class _GBuffer(C.Structure):
@@ -60,6 +64,10 @@ def load():
         lib.nbsdf_last_error.argtypes = [C.c_void_p]
         lib.nbsdf_launch_count.restype = C.c_int64
         lib.nbsdf_launch_count.argtypes = [C.c_void_p]
+        lib.nbsdf_create_paper.restype = C.c_int
+        lib.nbsdf_create_paper.argtypes = [C.POINTER(_Config), C.POINTER(_PaperWeights), C.POINTER(C.c_void_p)]
+        lib.nbsdf_set_albedos.restype = C.c_int
+        lib.nbsdf_set_albedos.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         _lib = lib
     return _lib
 
@@ -94,6 +102,30 @@ def nbsdf_create(weights, biases, latent_dim, hidden, max_materials, precision="
     rc = load().nbsdf_create(C.byref(cfg), C.byref(wt), C.byref(ctx))
     _check(rc, None)
     return ctx
+
+
+def nbsdf_create_paper(weights, biases, hidden, max_materials, precision="fp16", device=0, latent_dim=64, feat_dim=32):
+    """Paper-structured decoder (include/nbsdf.h): 7 host arrays each, W_k row-major [out][in] fp32."""
+    Ws = [np.ascontiguousarray(w, dtype=np.float32) for w in weights]
+    bs = [np.ascontiguousarray(b, dtype=np.float32).reshape(-1) for b in biases]
+    L, H, F = latent_dim, hidden, feat_dim
+    for w, b, s in zip(Ws, bs, [(H, L + 24), (F, H), (H, F + 5), (H, H), (H, H), (H, H), (4, H)]):
+        if w.shape != s or b.shape != (s[0],):
+            raise ValueError(f"layer shape {w.shape}/{b.shape}, expected {s}")
+    cfg = _Config(L, H, F, max_materials, PRECISIONS.get(precision, precision), device)
+    wt = _PaperWeights((C.c_void_p * 7)(*[w.ctypes.data for w in Ws]), (C.c_void_p * 7)(*[b.ctypes.data for b in bs]))
+    ctx = C.c_void_p()
+    rc = load().nbsdf_create_paper(C.byref(cfg), C.byref(wt), C.byref(ctx))
+    _check(rc, None)
+    return ctx
+
+
+def nbsdf_set_albedos(ctx, first, albedos_host, stream=None):
+    a = np.ascontiguousarray(albedos_host, dtype=np.float32)
+    a = a.reshape(1, -1) if a.ndim == 1 else a
+    if a.shape[1] != 12:
+        raise ValueError("albedos: 12 values per material (kd_warp, kd_weft, ks_warp, ks_weft) x RGB")
+    _check(load().nbsdf_set_albedos(ctx, first, a.shape[0], a.ctypes.data, _stream(stream)), ctx)
 
 
 def nbsdf_set_latents(ctx, first, latents_host, stream=None):

@@ -5,8 +5,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libnbsdf.so")
-SOURCES = ["nbsdf_host.cu", "nbsdf_fp32.cu", "nbsdf_tc.cu"]
-HEADERS = ["nbsdf_common.cuh", os.path.join("..", "..", "include", "nbsdf.h")]
+SOURCES = ["nbsdf_host.cu", "nbsdf_fp32.cu", "nbsdf_tc.cu", "nbsdf_tc_paper.cu"]
+HEADERS = ["nbsdf_common.cuh", "nbsdf_tc_ptx.cuh", os.path.join("..", "..", "include", "nbsdf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--threads", "0"]
 

@@ -17,6 +17,7 @@ struct NetParams {
     const float* w32;       // fp32 path: transposed, padded weights + biases (see pack_fp32)
     const uint8_t* wimg_eval;    // tensor path: shared-memory image for nbsdf_eval (5 layers, feature layer merged)
     const uint8_t* wimg_shade;   // tensor path: shared-memory image for nbsdf_shade_frame (6 layers)
+    const float* albedos;        // paper-structured decoder: [M][12] fp32 (kd_warp, kd_weft, ks_warp, ks_weft) x RGB
     int32_t L, H, M;
 };
 
@@ -197,5 +198,46 @@ __host__ __device__ constexpr TcLayout tc_layout(int L, int H, bool merged)
     t.total = (off + 15u) & ~15u;
     return t;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Paper-structured decoder (nbsdf_tc_paper.cu): seven layers, same image format as above.
+//   1: [z(64), blob(24), c] -> H     2: H -> F       (fusion)
+//   3: [feat(F), wi(3), wo(2), c] -> H   4: H -> H   5: H -> H (+ skip, added in the epilogue)   6: H -> H   7: H -> 4
+constexpr int kPdLatent = 64;
+constexpr int kPdBlob = 24;
+constexpr int kPdLayers = 7;
+constexpr float kPdSlope = 0.01f;
+
+struct PdLayout {
+    int Kp[kPdLayers];            // padded K as issued
+    int Kbias[kPdLayers];         // input index of the first bias column
+    uint32_t w_off[kPdLayers];
+    uint32_t w_rows[kPdLayers];   // padded N
+    uint32_t total;
+};
+
+__host__ __device__ constexpr PdLayout pd_layout(int H)
+{
+    PdLayout t{};
+    const int K[kPdLayers] = { pad16(kPdLatent + kPdBlob + kBiasCols), H + 16, pad16(kFeat + 5 + kBiasCols), H + 16, H + 16, H + 16, H + 16 };
+    const int Kb[kPdLayers] = { kPdLatent + kPdBlob, H, kFeat + 5, H, H, H, H };
+    const int N[kPdLayers] = { H, kFeat, H, H, H, H, 16 };
+    uint32_t off = 0;
+    for (int l = 0; l < kPdLayers; ++l) {
+        t.Kp[l] = K[l];
+        t.Kbias[l] = Kb[l];
+        t.w_off[l] = off;
+        t.w_rows[l] = (uint32_t)N[l];
+        off += (uint32_t)((K[l] + 63) / 64) * (uint32_t)N[l] * 128u;
+    }
+    t.total = (off + 15u) & ~15u;
+    return t;
+}
+
+cudaError_t init_pd(int H);
+cudaError_t launch_eval_pd(const NetParams& net, int precision, int num_sms, const nbsdf_query* q, const float* frames,
+                           int64_t n, float* rgb, cudaStream_t s);
+cudaError_t launch_shade_pd(const NetParams& net, int precision, int num_sms, const FrameParams& fr,
+                            const LightParams& lights, float* out, cudaStream_t s);
 
 }  // namespace nbsdf

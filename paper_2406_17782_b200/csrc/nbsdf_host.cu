@@ -28,6 +28,11 @@ struct nbsdf_ctx {
     float* h_stage = nullptr;         // pinned mirror used by set_latents
     cudaEvent_t stage_free = nullptr; // recorded after the last staged copy
     bool stage_busy = false;
+    int arch = 0;                     // 0: BASELINE.json decoder (nbsdf_create), 1: paper-structured (nbsdf_create_paper)
+    float* d_albedos = nullptr;       // arch 1: [M][12] fp32
+    float* h_alb = nullptr;           // pinned mirror used by set_albedos
+    cudaEvent_t alb_free = nullptr;
+    bool alb_busy = false;
     int64_t launches = 0;
     std::string err;
 };
@@ -184,10 +189,132 @@ extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weight
     return NBSDF_OK;
 }
 
+
+// Shared-memory image of the paper-structured decoder: same tile format as pack_tc, seven layers (pd_layout).
+static void pack_pd(int H, bool bf16, const nbsdf_paper_weights* w, uint8_t* img)
+{
+    const PdLayout lay = pd_layout(H);
+    const int F = kFeat;
+    const int Kr[kPdLayers] = { kPdLatent + kPdBlob, H, F + 5, H, H, H, H };
+    const int Nr[kPdLayers] = { H, F, H, H, H, H, 4 };
+    memset(img, 0, lay.total);
+    for (int l = 0; l < kPdLayers; ++l) {
+        const int Np = (int)lay.w_rows[l];
+        auto put = [&](int n, int k, uint16_t bits) {
+            const int kb = k / 64, kk = k % 64;
+            const int chunk = (kk / 8) ^ (n % 8);
+            const size_t off = lay.w_off[l] + (size_t)kb * Np * 128 + (size_t)n * 128 + (size_t)chunk * 16 + (size_t)(kk % 8) * 2;
+            memcpy(img + off, &bits, 2);
+        };
+        for (int n = 0; n < Nr[l]; ++n) {
+            for (int k = 0; k < Kr[l]; ++k) put(n, k, to_op16(w->W[l][(size_t)n * Kr[l] + k], bf16));
+            double r = (double)w->b[l][n];
+            for (int j = 0; j < kBiasCols; ++j) {       // three-way 16-bit split of the bias, as in pack_tc
+                const double c = (double)tc_bias_const(bf16, j);
+                const uint16_t bits = to_op16((float)(r / c), bf16);
+                put(n, lay.Kbias[l] + j, bits);
+                r -= (double)from_op16(bits, bf16) * c;
+            }
+        }
+    }
+}
+
+extern "C" int nbsdf_create_paper(const nbsdf_config* cfg, const nbsdf_paper_weights* weights, nbsdf_ctx** out)
+{
+    if (!cfg || !weights || !out) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create_paper: NULL argument");
+    *out = nullptr;
+    for (int l = 0; l < kPdLayers; ++l)
+        if (!weights->W[l] || !weights->b[l]) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create_paper: NULL weight or bias pointer");
+    if (cfg->precision < NBSDF_PREC_FP32 || cfg->precision > NBSDF_PREC_FP16)
+        return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create_paper: unknown precision");
+    if (cfg->precision == NBSDF_PREC_FP32 || cfg->latent_dim != kPdLatent || cfg->hidden != 64 || cfg->feat_dim != kFeat ||
+        cfg->max_materials < 1 || cfg->max_materials > 64)
+        return fail(nullptr, NBSDF_E_UNSUPPORTED,
+                    "nbsdf_create_paper: supported are latent_dim 64, hidden 64, feat_dim 32, 1..64 materials, fp16/bf16 operands");
+    int n_dev = 0;
+    cudaError_t e = cudaGetDeviceCount(&n_dev);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceCount", e);
+    if (cfg->device < 0 || cfg->device >= n_dev) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create_paper: no such device");
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, cfg->device);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceProperties", e);
+    if (prop.major != 10)
+        return fail(nullptr, NBSDF_E_UNSUPPORTED, "nbsdf_create_paper: device is not sm_100 (Blackwell B200); there is no fallback path");
+    e = cudaSetDevice(cfg->device);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaSetDevice", e);
+
+    nbsdf_ctx* ctx = new (std::nothrow) nbsdf_ctx();
+    if (!ctx) return fail(nullptr, NBSDF_E_NOMEM, "nbsdf_create_paper: out of host memory");
+    ctx->cfg = *cfg;
+    ctx->arch = 1;
+    ctx->num_sms = prop.multiProcessorCount;
+    const int L = cfg->latent_dim, H = cfg->hidden, M = cfg->max_materials;
+#define NBSDF_TRY(call, what)                                                    \
+    do {                                                                         \
+        cudaError_t e_ = (call);                                                 \
+        if (e_ != cudaSuccess) {                                                 \
+            int rc_ = fail_cuda(nullptr, what, e_);                              \
+            nbsdf_destroy(ctx);                                                  \
+            return e_ == cudaErrorMemoryAllocation ? NBSDF_E_NOMEM : rc_;        \
+        }                                                                        \
+    } while (0)
+    NBSDF_TRY(cudaMalloc(&ctx->d_latents, (size_t)M * L * sizeof(float)), "cudaMalloc(latents)");
+    NBSDF_TRY(cudaMemset(ctx->d_latents, 0, (size_t)M * L * sizeof(float)), "cudaMemset(latents)");
+    NBSDF_TRY(cudaMallocHost(&ctx->h_stage, (size_t)M * L * sizeof(float)), "cudaMallocHost(stage)");
+    NBSDF_TRY(cudaEventCreateWithFlags(&ctx->stage_free, cudaEventDisableTiming), "cudaEventCreate");
+    NBSDF_TRY(cudaMalloc(&ctx->d_albedos, (size_t)M * 12 * sizeof(float)), "cudaMalloc(albedos)");
+    NBSDF_TRY(cudaMemset(ctx->d_albedos, 0, (size_t)M * 12 * sizeof(float)), "cudaMemset(albedos)");
+    NBSDF_TRY(cudaMallocHost(&ctx->h_alb, (size_t)M * 12 * sizeof(float)), "cudaMallocHost(albedos)");
+    NBSDF_TRY(cudaEventCreateWithFlags(&ctx->alb_free, cudaEventDisableTiming), "cudaEventCreate");
+    {
+        const PdLayout lay = pd_layout(H);
+        std::vector<uint8_t> img(lay.total);
+        pack_pd(H, cfg->precision == NBSDF_PREC_BF16, weights, img.data());
+        NBSDF_TRY(cudaMalloc(&ctx->d_wimg_eval, lay.total), "cudaMalloc(wimg)");
+        NBSDF_TRY(cudaMemcpy(ctx->d_wimg_eval, img.data(), lay.total, cudaMemcpyHostToDevice), "cudaMemcpy(wimg)");
+        ctx->d_wimg_shade = ctx->d_wimg_eval;
+    }
+    NBSDF_TRY(init_pd(H), "cudaFuncSetAttribute(pd)");
+#undef NBSDF_TRY
+    *out = ctx;
+    return NBSDF_OK;
+}
+
+extern "C" int nbsdf_set_albedos(nbsdf_ctx* ctx, int32_t first, int32_t count, const float* albedos_host, void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (ctx->arch != 1) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: context was not made by nbsdf_create_paper");
+    if (first < 0 || count < 0 || (int64_t)first + count > ctx->cfg.max_materials)
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: rows out of range");
+    if (count == 0) return NBSDF_OK;
+    if (!albedos_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: NULL albedos");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSetDevice(ctx->cfg.device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    if (ctx->alb_busy) {
+        e = cudaEventSynchronize(ctx->alb_free);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventSynchronize", e);
+        ctx->alb_busy = false;
+    }
+    float* src = ctx->h_alb + (size_t)first * 12;
+    memcpy(src, albedos_host, (size_t)count * 12 * sizeof(float));
+    e = cudaMemcpyAsync(ctx->d_albedos + (size_t)first * 12, src, (size_t)count * 12 * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemcpyAsync(albedos)", e);
+    e = cudaEventRecord(ctx->alb_free, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
+    ctx->alb_busy = true;
+    return NBSDF_OK;
+}
+
 extern "C" void nbsdf_destroy(nbsdf_ctx* ctx)
 {
     if (!ctx) return;
     if (ctx->stage_busy && ctx->stage_free) cudaEventSynchronize(ctx->stage_free);
+    if (ctx->alb_busy && ctx->alb_free) cudaEventSynchronize(ctx->alb_free);
+    if (ctx->d_albedos) cudaFree(ctx->d_albedos);
+    if (ctx->h_alb) cudaFreeHost(ctx->h_alb);
+    if (ctx->alb_free) cudaEventDestroy(ctx->alb_free);
+    if (ctx->arch == 1) ctx->d_wimg_shade = nullptr;      // alias of d_wimg_eval
     if (ctx->d_latents) cudaFree(ctx->d_latents);
     if (ctx->d_w32) cudaFree(ctx->d_w32);
     if (ctx->d_wimg_eval) cudaFree(ctx->d_wimg_eval);
@@ -238,6 +365,7 @@ static NetParams net_params(const nbsdf_ctx* ctx)
     p.w32 = ctx->d_w32;
     p.wimg_eval = ctx->d_wimg_eval;
     p.wimg_shade = ctx->d_wimg_shade;
+    p.albedos = ctx->d_albedos;
     p.L = ctx->cfg.latent_dim;
     p.H = ctx->cfg.hidden;
     p.M = ctx->cfg.max_materials;
@@ -259,7 +387,8 @@ extern "C" int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float*
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
     const NetParams net = net_params(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_eval_fp32(net, q_dev, frames_dev, n, rgb_dev, s);
+    if (ctx->arch == 1) e = launch_eval_pd(net, ctx->cfg.precision, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
+    else if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_eval_fp32(net, q_dev, frames_dev, n, rgb_dev, s);
     else e = launch_eval_tc(net, ctx->cfg.precision, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_eval launch", e);
     ctx->launches += 1;
@@ -307,7 +436,8 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     fr.cam[0] = g->cam_pos[0]; fr.cam[1] = g->cam_pos[1]; fr.cam[2] = g->cam_pos[2];
     const NetParams net = net_params(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_shade_fp32(net, fr, lp, radiance_dev, s);
+    if (ctx->arch == 1) e = launch_shade_pd(net, ctx->cfg.precision, ctx->num_sms, fr, lp, radiance_dev, s);
+    else if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_shade_fp32(net, fr, lp, radiance_dev, s);
     else e = launch_shade_tc(net, ctx->cfg.precision, ctx->num_sms, fr, lp, radiance_dev, s);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_shade_frame launch", e);
     ctx->launches += 1;

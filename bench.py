@@ -149,6 +149,58 @@ def time_loop(torch, fn, steps, barrier):
     return e0.elapsed_time(e1)
 
 
+PD_FLOP_FUSION = 2 * (88 * 64 + 64 * 32)                                                # 15 360
+PD_FLOP_ANGULAR = 2 * (37 * 64 + 3 * 64 * 64 + 64 * 4)                                  # 29 824
+PD_FLOP_PER_QUERY = PD_FLOP_FUSION + PD_FLOP_ANGULAR                                    # 45 184, unpadded
+
+
+def measure_paper(torch, api, synth, dev, K, peaks, prec, seed_shift=0):
+    """the paper-structured decoder (nbsdf_create_paper) on the same two workload shapes --
+    2^20 Table-2 queries per launch, and the 1080p G-buffer with 5 direct lights + 1 light behind the fabric."""
+    n = 1 << 20
+    cfg = synth.pd_config("eval", n=n, seed=11 + seed_shift)
+    ctx = api.nbsdf_create_paper(cfg["weights"], cfg["biases"], 64, 8, prec, device=dev.index or 0)
+    api.nbsdf_set_latents(ctx, 0, cfg["latents"])
+    api.nbsdf_set_albedos(ctx, 0, cfg["albedos"])
+    qs = [torch.from_numpy(np.roll(cfg["queries"], r * 12345).view(np.uint8).reshape(-1).copy()).to(dev) for r in range(N_ROTATE)]
+    outs = [torch.empty((n, 3), dtype=torch.float32, device=dev) for _ in range(N_ROTATE)]
+    step = lambda i: api.nbsdf_eval(ctx, qs[i % N_ROTATE], None, n, outs[i % N_ROTATE])
+    for i in range(5):
+        step(i)
+    torch.cuda.synchronize()
+    k = max(3, min(K, 500))
+    ms = time_loop(torch, step, k, lambda: None) / k
+    fcfg = synth.pd_config("frame", seed=12 + seed_shift)
+    api.nbsdf_destroy(ctx)
+    fctx = api.nbsdf_create_paper(fcfg["weights"], fcfg["biases"], 64, 8, prec, device=dev.index or 0)
+    api.nbsdf_set_latents(fctx, 0, fcfg["latents"])
+    api.nbsdf_set_albedos(fctx, 0, fcfg["albedos"])
+    g = fcfg["gbuffer"]
+    npx = g["width"] * g["height"]
+    gds, rads = [], []
+    for r in range(3):
+        gr = {kk: np.roll(g[kk], r * 4099, axis=0) for kk in ("pos_fp", "nrm_u", "tan_v", "material")}
+        gr.update(width=g["width"], height=g["height"], cam_pos=g["cam_pos"])
+        gds.append(api.gbuffer_to_device(gr, dev))
+        rads.append(torch.empty((npx, 3), dtype=torch.float32, device=dev))
+    fstep = lambda i: api.nbsdf_shade_frame(fctx, gds[i % 3], fcfg["lights"], rads[i % 3])
+    for i in range(3):
+        fstep(i)
+    torch.cuda.synchronize()
+    kf = max(3, min(K, 200))
+    fms = time_loop(torch, fstep, kf, lambda: None) / kf
+    api.nbsdf_destroy(fctx)
+    n_l = len(fcfg["lights"])
+    tf = PD_FLOP_PER_QUERY * n / (ms * 1e-3) / 1e12
+    ftf = npx * (PD_FLOP_FUSION + n_l * PD_FLOP_ANGULAR) / (fms * 1e-3) / 1e12
+    return {"workload": "paper-structured decoder (latent 64, one-blob 24, 2 fusion + 5 angular layers, H=64, F=32): "
+                        "2^20 Table-2 queries per launch; 1920x1080 frame with 5 direct lights + 1 behind the fabric",
+            "queries_per_s": n / (ms * 1e-3), "us_per_launch": ms * 1e3, "flop_per_query": PD_FLOP_PER_QUERY,
+            "achieved_tflops": tf, "frac": tf / peaks["bf16_tflops"], "bound": "tensor",
+            "frame_ms": fms, "frame_lights": n_l, "frame_flop_per_pixel": PD_FLOP_FUSION + n_l * PD_FLOP_ANGULAR,
+            "frame_achieved_tflops": ftf, "frame_frac": ftf / peaks["bf16_tflops"], "steps": k, "frame_steps": kf}
+
+
 def run_ours(args):
     import torch
     from paper_2406_17782_b200 import api, dist, synth
@@ -244,6 +296,8 @@ def run_ours(args):
     torch.cuda.synchronize()
     fms = dist.max_over_ranks(time_loop(torch, fstep, kf, barrier), dev) / kf
 
+    paper = measure_paper(torch, api, synth, dev, K, peaks, prec) if (rank == 0 and prec != "fp32") else None
+
     line = None
     if rank == 0:
         us_per_launch = 1e3 * ms / K
@@ -288,6 +342,7 @@ def run_ours(args):
                       "frame_ms": fms, "steps": kf, "flop_per_pixel": FLOP_MLP_A + 5 * FLOP_MLP_B,
                       "achieved_tflops": frame_tf, "frac": frame_tf / peaks["bf16_tflops"] if prec != "fp32" else frame_tf / 74.4,
                       "decoder_evals_per_s": world * npx * 5 / (fms * 1e-3)},
+            "paper_decoder": paper,
             "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle", "value_1_thread": cpu_rate_1t,
                              "sample": f"first {n_cpu} of the 2^20 queries of configs[1], fp64, OpenMP over queries, {cpu_dt:.1f} s"},
         }

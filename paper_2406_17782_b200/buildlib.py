@@ -35,7 +35,7 @@ def build(force=False, verbose=False):
     for s in SOURCES:
         o = os.path.join(_HERE, "build", s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
+        cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("NBSDF_EXTRA_NVCC", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, p in procs:
         out, _ = p.communicate()

@@ -9,7 +9,7 @@
 // in the shadow of an MMA wait.  What differs:
 //   * seven MMA rounds per query (fusion 1-2 once per query / pixel, angular decoder 3-7 once per query / light);
 //   * round 1 reads K = 96 from two regions: z (64) from AH and [blob(24), c0, c1, c2] from AY;
-//   * the epilogue is a leaky ReLU (fp16 mode: on the packed pair, HMUL2 + HMNMX2; bf16 mode: in fp32) and round 5
+//   * the epilogue is a leaky ReLU (fp16 mode: on the packed pair with HMUL2 + HMNMX2; bf16 mode: in fp32) and round 5
 //     adds the skip connection from round 3's output, which the owning thread keeps as 32 packed registers;
 //   * the output stage inverts the log map of the two specular components and applies Eq. 8.
 //
@@ -40,6 +40,7 @@ struct Pd {
     static constexpr int kOwnerRegsRaw = kBaseRegs + kIssuerWarps * 32 * (kBaseRegs - kIssuerRegs) / (NWG * 128) / 8 * 8;
     static constexpr int kOwnerRegs = kOwnerRegsRaw > 248 ? 248 : kOwnerRegsRaw;
     static_assert(kThreads <= 1024, "CTA size");
+    static constexpr bool kTwoLoads = kOwnerRegs >= 136;          // epilogue register budget (see pd_epilogue)
 
     static constexpr uint32_t kLatBytes = 64 * kPdLatent * 2;     // packed latent table, max M x 64
     static constexpr uint32_t kAlbBytes = 64 * 12 * 4;            // albedo table, max M x 12 fp32
@@ -66,6 +67,7 @@ __device__ __forceinline__ uint32_t lrelu_pack(float lo, float hi, uint32_t skip
         hi = fmaxf(hi, kPdSlope * hi);
         return pack2<true, false>(lo, hi);
     } else {
+        // on the packed fp16 pair: one FMA-pipe and one ALU-pipe instruction next to the conversion
         uint32_t p = pack2<false, false>(lo, hi);
         __half2 h = *reinterpret_cast<__half2*>(&p);
         if constexpr (kSkip) h = __hadd2(h, *reinterpret_cast<const __half2*>(&skip));
@@ -76,9 +78,29 @@ __device__ __forceinline__ uint32_t lrelu_pack(float lo, float hi, uint32_t skip
 
 // Epilogue of a hidden layer: acc (N fp32 columns, bias inside) -> leaky ReLU -> packed pairs -> A columns.
 // kMode 0: plain; 1: also keep the packed result in skip[] (round 3); 2: add skip[] before the activation (round 5).
-template <int N, int kMode, bool kBf16>
+template <int N, int kMode, bool kBf16, bool kTwoLoads = false>
 __device__ __forceinline__ void pd_epilogue(uint32_t acc_taddr, uint32_t a_taddr, uint32_t (&skip)[32])
 {
+    if constexpr (kTwoLoads && N == 64) {
+        uint32_t v[32], w[32];
+        tmem_ld32(acc_taddr, v);
+        tmem_ld32(acc_taddr + 32, w);
+        tmem_wait_ld();
+        uint32_t p[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            p[j] = lrelu_pack<kBf16, kMode == 2>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]), skip[j]);
+            if (kMode == 1) skip[j] = p[j];
+        }
+        tmem_st16(a_taddr, p);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            p[j] = lrelu_pack<kBf16, kMode == 2>(__uint_as_float(w[2 * j]), __uint_as_float(w[2 * j + 1]), skip[16 + j]);
+            if (kMode == 1) skip[16 + j] = p[j];
+        }
+        tmem_st16(a_taddr + 16, p);
+        return;
+    }
 #pragma unroll
     for (int c = 0; c < N; c += 32) {
         uint32_t v[32];
@@ -450,7 +472,7 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         // ---- fusion ----
         publish();                                        // -> round 1
         await_mma();
-        pd_epilogue<H, 0, kBf16>(acc_t, ah_t, skip);
+        pd_epilogue<H, 0, kBf16, T::kTwoLoads>(acc_t, ah_t, skip);
         publish();                                        // -> round 2
         flush_output();                                   // shadow: the previous tile's output stage
         if constexpr (kShade) light_tail(0);              //         and C1 of the first light
@@ -477,11 +499,11 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 }
             }
             await_mma();
-            pd_epilogue<H, 1, kBf16>(acc_t, ah_t, skip);  // D1, kept for the skip connection
+            pd_epilogue<H, 1, kBf16, T::kTwoLoads>(acc_t, ah_t, skip);  // D1, kept for the skip connection
             publish();                                    // -> round 4
             if constexpr (!kShade) assemble(tile + stride, k + 1u);     // shadow: A1-A4 of the next tile (AY is dead)
             await_mma();
-            pd_epilogue<H, 0, kBf16>(acc_t, ah_t, skip);
+            pd_epilogue<H, 0, kBf16, T::kTwoLoads>(acc_t, ah_t, skip);
             publish();                                    // -> round 5; eval: the issuer also refills the staging buffer just read
             if constexpr (kShade) {                       // shadow: C1 of the next light, or A1-A4 of the next tile
                 if (l + 1 < n_rounds) {
@@ -492,10 +514,10 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 }
             }
             await_mma();
-            pd_epilogue<H, 2, kBf16>(acc_t, ah_t, skip);  // + skip, then leaky ReLU
+            pd_epilogue<H, 2, kBf16, T::kTwoLoads>(acc_t, ah_t, skip);  // + skip, then leaky ReLU
             publish();                                    // -> round 6
             await_mma();
-            pd_epilogue<H, 0, kBf16>(acc_t, ah_t, skip);
+            pd_epilogue<H, 0, kBf16, T::kTwoLoads>(acc_t, ah_t, skip);
             publish();                                    // -> round 7
             await_mma();
             load_output();
@@ -518,7 +540,13 @@ template <int H, bool kBf16, bool kShade>
 static cudaError_t pd_launch_one(const NetParams& net, int num_sms, const nbsdf_query* q, const float* frames, int64_t n,
                                  const FrameParams& fr, const LightParams& lights, float* out, cudaStream_t s, bool init_only)
 {
-    constexpr int NWG = 4;
+#ifndef NBSDF_PD_NWG_EVAL
+#define NBSDF_PD_NWG_EVAL 4
+#endif
+#ifndef NBSDF_PD_NWG_SHADE
+#define NBSDF_PD_NWG_SHADE 3
+#endif
+    constexpr int NWG = kShade ? NBSDF_PD_NWG_SHADE : NBSDF_PD_NWG_EVAL;
     using T = Pd<H, kBf16, NWG, kShade>;
     auto kern = pd_kernel<H, kBf16, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());

@@ -93,14 +93,19 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def oracle_rate(cfg, n_sample, threads=0):
-    """queries/s of the fp64 oracle, as it stands, on the first n_sample queries of cfg."""
+def oracle_rate(cfg, n_sample, threads=0, min_seconds=0.0):
+    """queries/s of the fp64 oracle, as it stands, on the first n_sample queries of cfg; the pass is repeated until
+    min_seconds of CPU work have been timed.  Returns (rate, seconds, passes)."""
     import oracle
     q = cfg["queries"][:n_sample]
     t0 = time.perf_counter()
-    oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], q, n_threads=threads)
-    dt = time.perf_counter() - t0
-    return len(q) / dt, dt
+    passes = 0
+    while True:
+        oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], q, n_threads=threads)
+        passes += 1
+        dt = time.perf_counter() - t0
+        if dt >= min_seconds:
+            return passes * len(q) / dt, dt, passes
 
 
 def run_reference(args):
@@ -112,7 +117,7 @@ def run_reference(args):
     import oracle
     cores = len(os.sched_getaffinity(0))
     cfg = synth.config(1, n=1 << 18)
-    rate0, _ = oracle_rate(cfg, 1 << 13)
+    rate0, _, _ = oracle_rate(cfg, 1 << 13)
     budget_s = 150.0
     n_step = int(min(1 << 18, max(256, rate0 * budget_s / max(1, args.steps + args.warmup))))
     for _ in range(args.warmup):
@@ -313,8 +318,8 @@ def run_ours(args):
         frame_tf = frame_flop / (fms * 1e-3) / 1e12
         cores = len(os.sched_getaffinity(0))
         n_cpu = 1 << 20
-        cpu_rate, cpu_dt = oracle_rate(cfg, n_cpu)
-        cpu_rate_1t, _ = oracle_rate(cfg, 1 << 16, threads=1)
+        cpu_rate, cpu_dt, cpu_passes = oracle_rate(cfg, n_cpu, min_seconds=12.0)
+        cpu_rate_1t, _, _ = oracle_rate(cfg, 1 << 16, threads=1, min_seconds=2.0)
         import oracle
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -344,7 +349,7 @@ def run_ours(args):
                       "decoder_evals_per_s": world * npx * 5 / (fms * 1e-3)},
             "paper_decoder": paper,
             "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle", "value_1_thread": cpu_rate_1t,
-                             "sample": f"first {n_cpu} of the 2^20 queries of configs[1], fp64, OpenMP over queries, {cpu_dt:.1f} s"},
+                             "sample": f"all {n_cpu} queries of configs[1], {cpu_passes} passes, fp64, OpenMP over queries, {cpu_dt:.1f} s"},
         }
     api.nbsdf_destroy(ctx)
     api.nbsdf_destroy(fctx)

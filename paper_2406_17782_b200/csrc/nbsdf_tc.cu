@@ -29,6 +29,9 @@
 #ifndef NBSDF_NWG64_EVAL
 #define NBSDF_NWG64_EVAL 4
 #endif
+#ifndef NBSDF_NWG64_SHADE
+#define NBSDF_NWG64_SHADE 4
+#endif
 
 namespace nbsdf {
 
@@ -68,7 +71,7 @@ struct Tc {
     static constexpr int kOwnerRegsRaw = kBaseRegs + kIssuerWarps * 32 * (kBaseRegs - kIssuerRegs) / (NWG * 128) / 8 * 8;
     static constexpr int kOwnerRegs = kOwnerRegsRaw > 248 ? 248 : kOwnerRegsRaw;
     static_assert(kThreads <= 1024, "CTA size");
-    static constexpr bool kTwoLoads = kOwnerRegs >= (kShade ? 160 : 100);         // epilogue register budget (see epilogue_to_a)
+    static constexpr bool kTwoLoads = kOwnerRegs >= (kShade ? 150 : 100);         // epilogue register budget (see epilogue_to_a)
     // TMEM columns of one warpgroup.  eval: x, the hidden activations and y share ONE A-operand region (each is dead
     // before the next is written); shade: y = [feat, wi, wo] must survive the light loop, so it gets its own region.
     // Merged eval adds an 8-column tail block [wi, wo, c0, c1, c2, 0...]: the last K step of the merged layer.
@@ -599,7 +602,7 @@ template <int L, int H, bool kBf16, bool kShade>
 static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_query* q, const float* frames, int64_t n,
                               const FrameParams& fr, const LightParams& lights, float* out, cudaStream_t s, bool init_only)
 {
-    constexpr int NWG = H == 128 ? 2 : (H == 32 ? (kShade ? 5 : NBSDF_NWG32_EVAL) : (kShade ? 4 : NBSDF_NWG64_EVAL));
+    constexpr int NWG = H == 128 ? 2 : (H == 32 ? (kShade ? 5 : NBSDF_NWG32_EVAL) : (kShade ? NBSDF_NWG64_SHADE : NBSDF_NWG64_EVAL));
     using T = Tc<L, H, kBf16, NWG, kShade>;
     auto kern = tc_kernel<L, H, kBf16, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());

@@ -30,16 +30,29 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
-// Waits for the phase with the given parity.  A wait that lasts ~seconds means a broken pipeline: trap instead of
-// hanging the GPU.
+// Waits for the phase with the given parity: a two-instruction retry loop around try_wait (which itself suspends
+// the warp for a hardware-defined time).  The loop is bounded -- 2^24 failed tries is seconds, i.e. a broken
+// pipeline -- and traps instead of hanging the GPU.  Every instruction here competes with the epilogues for issue
+// slots, so the loop carries no clock reads.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    if (mbar_try_wait(bar, parity)) return;
-    const long long t0 = clock64();
-    uint32_t spins = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) __trap();
-    }
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .u32 n;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "mov.u32 n, 0;\n"
+        "RETRY_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "add.u32 n, n, 1;\n\t"
+        "setp.lt.u32 p, n, 16777216;\n\t"
+        "@p bra RETRY_%=;\n\t"
+        "trap;\n"
+        "DONE_%=:\n\t"
+        "}"
+        ::"r"(bar), "r"(parity) : "memory");
 }
 // 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)

@@ -42,7 +42,9 @@ struct Pd {
     static_assert(kThreads <= 1024, "CTA size");
     static constexpr bool kTwoLoads = kOwnerRegs >= 136;          // epilogue register budget (see pd_epilogue)
 
-    static constexpr uint32_t kLatBytes = 64 * kPdLatent * 2;     // packed latent table, max M x 64
+    static constexpr uint32_t kLatRow = kPdLatent * 2 + 16;       // bytes per packed latent row: 16 bytes of padding put
+                                                                  // rows of different materials in different banks
+    static constexpr uint32_t kLatBytes = 64 * kLatRow;           // packed latent table, max M rows
     static constexpr uint32_t kAlbBytes = 64 * 12 * 4;            // albedo table, max M x 12 fp32
     static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);
     static constexpr uint32_t kStages = 2;
@@ -116,6 +118,13 @@ __device__ __forceinline__ void pd_epilogue(uint32_t acc_taddr, uint32_t a_taddr
     }
 }
 
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // e^y - 1 for the inverse log map (fast path: ex2 on the special-function unit; series near 0 where it cancels)
 __device__ __forceinline__ float fast_expm1(float y)
 {
@@ -184,7 +193,8 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         uint16_t* lat = reinterpret_cast<uint16_t*>(g_lat);
         for (int i = tid; i < net.M * L; i += T::kThreads) {
             const float z = __ldg(net.latents + i);
-            lat[i] = kBf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(z)) : __half_as_ushort(__float2half_rn(z));
+            lat[(i / L) * (T::kLatRow / 2) + (i % L)] =
+                kBf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(z)) : __half_as_ushort(__float2half_rn(z));
         }
         for (int i = tid; i < net.M * 12; i += T::kThreads) g_alb[i] = __ldg(net.albedos + i);
     }
@@ -383,11 +393,12 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         uint32_t xb[16];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            const float s8 = 8.0f * sc[a];
+            // distances pre-scaled by sqrt(log2(e)/2) = 0.84932180: one FFMA, one FMUL, one MUFU.EX2 per channel
+            const float s8 = 6.7945744f * sc[a];
 #pragma unroll
             for (int i = 0; i < 8; i += 2) {
-                const float d0 = ((float)i + 0.5f) - s8, d1 = ((float)i + 1.5f) - s8;
-                xb[a * 4 + i / 2] = pack2<kBf16, false>(exp2f(-0.72134752f * d0 * d0), exp2f(-0.72134752f * d1 * d1));
+                const float d0 = ((float)i + 0.5f) * 0.84932180f - s8, d1 = ((float)i + 1.5f) * 0.84932180f - s8;
+                xb[a * 4 + i / 2] = pack2<kBf16, false>(ex2_approx(-d0 * d0), ex2_approx(-d1 * d1));
             }
         }
         xb[12] = c01; xb[13] = c2z; xb[14] = 0u; xb[15] = 0u;
@@ -459,7 +470,7 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 
         // ---- z -> AH (the previous tile's last layer has completed; [blob, c] is already in AY) ----
         {
-            const uint4* zrow = reinterpret_cast<const uint4*>(g_lat + (size_t)(mat_cur < 0 ? 0 : mat_cur) * L * 2);
+            const uint4* zrow = reinterpret_cast<const uint4*>(g_lat + (size_t)(mat_cur < 0 ? 0 : mat_cur) * T::kLatRow);
             uint32_t z[32];
 #pragma unroll
             for (int i = 0; i < 8; ++i) {

@@ -80,7 +80,11 @@ struct Tc {
     static constexpr int kAhCol = H;
     static constexpr int kAyCol = kShade ? H + H / 2 : H;
     static constexpr int kTailCol = H + kAw;
-    static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw + (kMerged ? 8 : 0);
+    // merged eval, when the columns are there: x gets a region of its own (read by layer 1 only), so that the input
+    // assembly of the next tile stores x and the tail block straight to TMEM and a tile starts without any store
+    static constexpr bool kXDirect = kMerged && NWG * (H + kAw + 8 + K1p / 2) <= 504;
+    static constexpr int kXCol = H + kAw + 8;
+    static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw + (kMerged ? 8 : 0) + (kXDirect ? K1p / 2 : 0);
     static constexpr int kOneCol = 504;              // CTA-wide constant block (c0, c1, c2, 0...): bias K step of the K = H layers
     static_assert(NWG * kColsPerWg <= kOneCol, "TMEM budget");
     static_assert(L % 8 == 0 && H % 32 == 0, "dims");
@@ -294,7 +298,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                     stage_request(first + 2 * stride, 2u);    // buffer 0 has been read by every thread of the warpgroup
                     mbar_wait(w_bar, 0);
                 }
-                issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, ay_d, one_d, w_s[0], mma_bar);
+                issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, T::kXDirect ? col0 + T::kXCol : ay_d, one_d, w_s[0], mma_bar);
             }
             __syncwarp();
             ready();
@@ -304,14 +308,18 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 ready();
                 if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, col0 + T::kTailCol, w_s[2], mma_bar);
                 __syncwarp();
-                ready();                                      // follows assemble(next): staging buffer (k + 1) & 1 is free
+                // the ready() that follows assemble(next) (one round later with kXDirect): staging buffer (k + 1) & 1 is free
+                ready();
                 if (elect_one()) {
-                    stage_request(tile + 3 * stride, k + 3u);
+                    if (!T::kXDirect) stage_request(tile + 3 * stride, k + 3u);
                     issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[3], mma_bar);
                 }
                 __syncwarp();
                 ready();
-                if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                if (elect_one()) {
+                    if (T::kXDirect) stage_request(tile + 3 * stride, k + 3u);
+                    issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                }
                 __syncwarp();
             } else {
                 ready();
@@ -425,6 +433,12 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 #pragma unroll
             for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
         }
+        if constexpr (T::kXDirect) {    // called after the merged layer has completed: x region and tail block are dead
+#pragma unroll
+            for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(lane_taddr + T::kXCol + i, x + i);
+            uint32_t y[8] = { ytail[0], ytail[1], ytail[2], c01, c2z, 0u, 0u, 0u };
+            tmem_st8(lane_taddr + T::kTailCol, y);
+        }
     };
 
     // shade, stage C1: geometry of light l at this pixel -> packed [wi_local, wo_local] and E * cos
@@ -488,11 +502,11 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         const int kind = item < n_items ? (material < 0 ? 2 : 1) : 0;
 
         // ---- layer-1 operand (and the merged layer's tail block) -> TMEM ----
-        if constexpr (!kShade) {
+        if constexpr (!kShade && !T::kXDirect) {
 #pragma unroll
             for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
         }
-        if constexpr (T::kMerged) store_tail(lane_taddr + T::kTailCol);
+        if constexpr (T::kMerged && !T::kXDirect) store_tail(lane_taddr + T::kTailCol);
         NBSDF_PHASE(0);
 
         // ---- MLP-A (B1-B3) ----
@@ -516,13 +530,14 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             // ---- merged layers 3+4 (B3-B4): (W4f W3) h2 + W4a [wi, wo] + (W4f b3 + b4); K = H from AH + tail block ----
             publish();                                    // -> merged layer
             NBSDF_PHASE(8);
-            assemble(tile + stride, k + 1u);              // shadow of the merged layer: A1-A4 of the next tile
+            if constexpr (!T::kXDirect) assemble(tile + stride, k + 1u);      // shadow of the merged layer: A1-A4 of the next tile
             NBSDF_PHASE(12);
             await_mma();
             NBSDF_PHASE(9);
             epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
             NBSDF_PHASE(10);
-            publish();                                    // -> layer 5; the issuer also refills the staging buffer just read
+            publish();                                    // -> layer 5
+            if constexpr (T::kXDirect) assemble(tile + stride, k + 1u);       // shadow of layer 5 (the merged layer is done)
             NBSDF_PHASE(11);
             await_mma();
             NBSDF_PHASE(13);

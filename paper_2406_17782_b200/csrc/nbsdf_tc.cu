@@ -311,14 +311,14 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 // the ready() that follows assemble(next) (one round later with kXDirect): staging buffer (k + 1) & 1 is free
                 ready();
                 if (elect_one()) {
-                    if (!T::kXDirect) stage_request(tile + 3 * stride, k + 3u);
                     issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[3], mma_bar);
+                    if (!T::kXDirect) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
                 }
                 __syncwarp();
                 ready();
                 if (elect_one()) {
-                    if (T::kXDirect) stage_request(tile + 3 * stride, k + 3u);
                     issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                    if (T::kXDirect) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
                 }
                 __syncwarp();
             } else {
@@ -332,8 +332,8 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                     __syncwarp();
                     ready();                                  // eval: follows assemble(next)
                     if (elect_one()) {
-                        if (!kShade) stage_request(tile + 3 * stride, k + 3u);
                         issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                        if (!kShade) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
                     }
                     __syncwarp();
                     ready();

@@ -286,8 +286,8 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 __syncwarp();
                 ready();                                          // eval: follows assemble(next): staging buffer (k + 1) & 1 is free
                 if (elect_one()) {
-                    if (!kShade) stage_request(tile + 3 * stride, k + 3u);
                     issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
+                    if (!kShade) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
                 }
                 __syncwarp();
                 ready();

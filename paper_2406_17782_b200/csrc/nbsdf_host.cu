@@ -379,6 +379,7 @@ extern "C" int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float*
 {
     if (!ctx) return NBSDF_E_INVALID;
     if (n < 0) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: negative n");
+    if (n >= ((int64_t)1 << 38)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: n must be below 2^38 per call");
     if (n == 0) return NBSDF_OK;
     if (!q_dev || !rgb_dev) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: NULL buffer");
     if (!aligned16(q_dev) || !aligned16(rgb_dev) || (frames_dev && (reinterpret_cast<uintptr_t>(frames_dev) & 7u)))

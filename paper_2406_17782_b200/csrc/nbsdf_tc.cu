@@ -233,20 +233,24 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     for (int l = 0; l < 6; ++l) w_s[l] = s_wimg + (l < lay.n_layers ? lay.w_off[l] : 0u);
 
     const int64_t n_items = kShade ? fr.n_pixels : n;
-    const int64_t n_tiles = (n_items + 127) / 128;
-    const int64_t stride = (int64_t)gridDim.x * NWG;
-    const int64_t first = (int64_t)blockIdx.x * NWG + wg;
+    // tile indices are 32-bit (the host rejects n >= 2^38); only addresses are formed in 64 bits
+    const int n_tiles = (int)((n_items + 127) / 128);
+    const int n_full = (int)(n_items / 128);                         // tiles [0, n_full) are complete
+    const int last_rows = (int)(n_items - (int64_t)n_full * 128);    // live rows of the ragged tile n_full, if any
+    const int stride = (int)gridDim.x * NWG;
+    const int first = (int)blockIdx.x * NWG + wg;
+    auto row_is_live = [&](int tile) { return tile < n_full || (tile == n_full && t < last_rows); };
     uint32_t mma_phase = 0;
     const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStages * T::kStageBytes;
     const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStages * T::kStageBytes;
 
     // eval: full tiles are staged in shared memory by bulk copies, two buffers per warpgroup; the tile processed in
     // iteration k of this warpgroup lives in buffer k & 1 and completes phase (k >> 1) & 1 of that buffer's mbarrier.
-    auto tile_is_bulk = [&](int64_t tile) { return !kShade && tile < n_tiles && (tile + 1) * 128 <= n_items; };
-    auto stage_request = [&](int64_t tile, uint32_t k) {      // one elected lane
+    auto tile_is_bulk = [&](int tile) { return !kShade && tile < n_full; };
+    auto stage_request = [&](int tile, uint32_t k) {      // one elected lane
         if (tile_is_bulk(tile)) {
             mbar_expect_tx(q_bar + 8u * (k & 1u), T::kStageBytes);
-            bulk_g2s(my_stage + (k & 1u) * T::kStageBytes, q + tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
+            bulk_g2s(my_stage + (k & 1u) * T::kStageBytes, q + (int64_t)tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
         }
     };
 
@@ -296,7 +300,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             tc_fence_after();
         };
         uint32_t k = 0;
-        for (int64_t tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
+        for (int tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
             ready();
             if (elect_one()) {
                 if (k == 0) {
@@ -355,11 +359,11 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     // (52 B/pixel, perfectly coalesced float4 planes)
     float4 pf_pos = make_float4(0.f, 0.f, 0.f, 1.f), pf_nu = make_float4(0.f, 0.f, 1.f, 0.f), pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
     int pf_mat = -1;
-    auto gbuf_request = [&](int64_t tile) {
-        const int64_t it = tile * 128 + t;
+    auto gbuf_request = [&](int tile) {
+        const int64_t it = (int64_t)tile * 128 + t;
         pf_pos = make_float4(0.f, 0.f, 0.f, 1.f); pf_nu = make_float4(0.f, 0.f, 1.f, 0.f); pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
         pf_mat = -1;
-        if (tile < n_tiles && it < n_items) {
+        if (row_is_live(tile)) {
             pf_pos = __ldg(fr.pos_fp + it); pf_nu = __ldg(fr.nrm_u + it); pf_tv = __ldg(fr.tan_v + it);
             pf_mat = __ldg(fr.material + it);
         }
@@ -375,15 +379,15 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     for (int c = 0; c < 3; ++c) { f.t[c] = c == 0; f.b[c] = c == 1; f.n[c] = c == 2; }
 
     // stages A1-A4 for `tile` (iteration k of this warpgroup): fetch + assemble into the state above
-    auto assemble = [&](int64_t tile, uint32_t k) {
-        const int64_t it = tile * 128 + t;
+    auto assemble = [&](int tile, uint32_t k) {
+        const int64_t it = (int64_t)tile * 128 + t;
         float up, vp, lf;
         if constexpr (!kShade) {
             nbsdf_query rec;
             rec.u = rec.v = 0.0f; rec.footprint = 1.0f; rec.material = -1;
             rec.wi[0] = rec.wi[1] = 0.0f; rec.wi[2] = 1.0f; rec.wo[0] = rec.wo[1] = 0.0f; rec.wo[2] = 1.0f;
             const bool bulk = tile_is_bulk(tile);
-            const bool direct = !bulk && tile < n_tiles && it < n_items;
+            const bool direct = !bulk && row_is_live(tile);
             auto unpack = [&](const uint2 w0, const uint2 w1, const uint2 w2, const uint2 w3, const uint2 w4) {
                 rec.u = __uint_as_float(w0.x); rec.v = __uint_as_float(w0.y);
                 rec.footprint = __uint_as_float(w1.x); rec.material = (int)w1.y;
@@ -467,7 +471,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 
     // deferred output of the tile finished last: raw output-layer values, their item and what to do with them
     float o_prev[3] = { 0.0f, 0.0f, 0.0f }, rad[3] = { 0.0f, 0.0f, 0.0f };
-    int64_t prev_item = 0;
+    int prev_tile = 0;
     int prev_kind = 0;                  // 0: nothing pending / dead row, 1: store, 2: background (store zeros)
     auto flush_output = [&]() {
         if (prev_kind != 0) {
@@ -478,9 +482,10 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 r[c] = kShade ? fmaf(v, w_cur[c], rad[c]) : v;
                 if (prev_kind == 2) r[c] = 0.0f;
             }
-            out[3 * prev_item + 0] = r[0];
-            out[3 * prev_item + 1] = r[1];
-            out[3 * prev_item + 2] = r[2];
+            float* o3 = out + 3 * ((int64_t)prev_tile * 128 + t);
+            o3[0] = r[0];
+            o3[1] = r[1];
+            o3[2] = r[2];
         }
         prev_kind = 0;
         rad[0] = rad[1] = rad[2] = 0.0f;
@@ -502,9 +507,8 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     for (int i = 0; i < 24; ++i) ph_acc[i] = 0;
 #endif
     uint32_t k = 0;
-    for (int64_t tile = first; tile < n_tiles; tile += stride, ++k) {
-        const int64_t item = tile * 128 + t;
-        const int kind = item < n_items ? (material < 0 ? 2 : 1) : 0;
+    for (int tile = first; tile < n_tiles; tile += stride, ++k) {
+        const int kind = row_is_live(tile) ? (material < 0 ? 2 : 1) : 0;
 
         // ---- layer-1 operand (and the merged layer's tail block) -> TMEM ----
         if constexpr (!kShade && !T::kXDirect) {
@@ -595,7 +599,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 load_output();
             }
         }
-        prev_item = item;
+        prev_tile = tile;
         prev_kind = kind;
     }
     flush_output();

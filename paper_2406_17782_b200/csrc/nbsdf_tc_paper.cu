@@ -211,20 +211,24 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     for (int l = 0; l < kPdLayers; ++l) w_s[l] = s_wimg + lay.w_off[l];
 
     const int64_t n_items = kShade ? fr.n_pixels : n;
-    const int64_t n_tiles = (n_items + 127) / 128;
-    const int64_t stride = (int64_t)gridDim.x * NWG;
-    const int64_t first = (int64_t)blockIdx.x * NWG + wg;
+    // tile indices are 32-bit (the host rejects n >= 2^38); only addresses are formed in 64 bits
+    const int n_tiles = (int)((n_items + 127) / 128);
+    const int n_full = (int)(n_items / 128);                         // tiles [0, n_full) are complete
+    const int last_rows = (int)(n_items - (int64_t)n_full * 128);    // live rows of the ragged tile n_full, if any
+    const int stride = (int)gridDim.x * NWG;
+    const int first = (int)blockIdx.x * NWG + wg;
+    auto row_is_live = [&](int tile) { return tile < n_full || (tile == n_full && t < last_rows); };
     uint32_t mma_phase = 0;
     const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStages * T::kStageBytes;
     const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStages * T::kStageBytes;
     const int n_rounds = kShade ? lights.n : 1;
 
     // eval: full tiles are staged by bulk copies, two buffers per warpgroup (see nbsdf_tc.cu)
-    auto tile_is_bulk = [&](int64_t tile) { return !kShade && tile < n_tiles && (tile + 1) * 128 <= n_items; };
-    auto stage_request = [&](int64_t tile, uint32_t k) {      // one elected lane
+    auto tile_is_bulk = [&](int tile) { return !kShade && tile < n_full; };
+    auto stage_request = [&](int tile, uint32_t k) {      // one elected lane
         if (tile_is_bulk(tile)) {
             mbar_expect_tx(q_bar + 8u * (k & 1u), T::kStageBytes);
-            bulk_g2s(my_stage + (k & 1u) * T::kStageBytes, q + tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
+            bulk_g2s(my_stage + (k & 1u) * T::kStageBytes, q + (int64_t)tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
         }
     };
     auto publish = [&]() {
@@ -269,7 +273,7 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             tc_fence_after();
         };
         uint32_t k = 0;
-        for (int64_t tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
+        for (int tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
             ready();                                              // round 1: z from AH (K 0..63), [blob, c] from AY (K 64..95)
             if (elect_one()) {
                 if (k == 0) {
@@ -310,11 +314,11 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     // shade: G-buffer texel prefetched one tile ahead into registers
     float4 pf_pos = make_float4(0.f, 0.f, 0.f, 1.f), pf_nu = make_float4(0.f, 0.f, 1.f, 0.f), pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
     int pf_mat = -1;
-    auto gbuf_request = [&](int64_t tile) {
-        const int64_t it = tile * 128 + t;
+    auto gbuf_request = [&](int tile) {
+        const int64_t it = (int64_t)tile * 128 + t;
         pf_pos = make_float4(0.f, 0.f, 0.f, 1.f); pf_nu = make_float4(0.f, 0.f, 1.f, 0.f); pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
         pf_mat = -1;
-        if (tile < n_tiles && it < n_items) {
+        if (row_is_live(tile)) {
             pf_pos = __ldg(fr.pos_fp + it); pf_nu = __ldg(fr.nrm_u + it); pf_tv = __ldg(fr.tan_v + it);
             pf_mat = __ldg(fr.material + it);
         }
@@ -344,15 +348,15 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 
     // Stages A1-A4 for `tile` (iteration k): fetch, wrap, one-blob encode -> AY columns [0, 16) = [blob(24), c0, c1, c2, 0...].
     // Only called when AY is dead: round 3 of the current tile (its last light) has completed.
-    auto assemble = [&](int64_t tile, uint32_t k) {
-        const int64_t it = tile * 128 + t;
+    auto assemble = [&](int tile, uint32_t k) {
+        const int64_t it = (int64_t)tile * 128 + t;
         float up, vp, size;
         if constexpr (!kShade) {
             nbsdf_query rec;
             rec.u = rec.v = 0.0f; rec.footprint = 1.0f; rec.material = -1;
             rec.wi[0] = rec.wi[1] = 0.0f; rec.wi[2] = 1.0f; rec.wo[0] = rec.wo[1] = 0.0f; rec.wo[2] = 1.0f;
             const bool bulk = tile_is_bulk(tile);
-            const bool direct = !bulk && tile < n_tiles && it < n_items;
+            const bool direct = !bulk && row_is_live(tile);
             auto unpack = [&](const uint2 w0, const uint2 w1, const uint2 w2, const uint2 w3, const uint2 w4) {
                 rec.u = __uint_as_float(w0.x); rec.v = __uint_as_float(w0.y);
                 rec.footprint = __uint_as_float(w1.x); rec.material = (int)w1.y;
@@ -434,7 +438,7 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         rgb[1] = a0.y * cw + a1.x * cf + a1.w * sw + a2.z * sf;
         rgb[2] = a0.z * cw + a1.y * cf + a2.x * sw + a2.w * sf;
     };
-    int64_t prev_item = 0;
+    int prev_tile = 0;
     int prev_kind = 0, prev_mat = 0;    // kind 0: nothing pending / dead row, 1: store, 2: background (store zeros)
     auto flush_output = [&]() {
         if (prev_kind != 0) {
@@ -445,9 +449,10 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 if (kShade) r[c] = fmaf(r[c], w_cur[c], rad[c]);
                 if (prev_kind == 2) r[c] = 0.0f;
             }
-            out[3 * prev_item + 0] = r[0];
-            out[3 * prev_item + 1] = r[1];
-            out[3 * prev_item + 2] = r[2];
+            float* o3 = out + 3 * ((int64_t)prev_tile * 128 + t);
+            o3[0] = r[0];
+            o3[1] = r[1];
+            o3[2] = r[2];
         }
         prev_kind = 0;
         rad[0] = rad[1] = rad[2] = 0.0f;
@@ -468,10 +473,9 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     if (first < n_tiles) assemble(first, 0u);
 
     uint32_t k = 0;
-    for (int64_t tile = first; tile < n_tiles; tile += stride, ++k) {
-        const int64_t item = tile * 128 + t;
+    for (int tile = first; tile < n_tiles; tile += stride, ++k) {
         const int mat_cur = material;
-        const int kind = item < n_items ? (mat_cur < 0 ? 2 : 1) : 0;
+        const int kind = row_is_live(tile) ? (mat_cur < 0 ? 2 : 1) : 0;
 
         // ---- z -> AH (the previous tile's last layer has completed; [blob, c] is already in AY) ----
         {
@@ -538,7 +542,7 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             await_mma();
             load_output();
         }
-        prev_item = item;
+        prev_tile = tile;
         prev_kind = kind;
         prev_mat = mat_cur;
     }

@@ -301,6 +301,24 @@ def run_ours(args):
     torch.cuda.synchronize()
     fms = dist.max_over_ranks(time_loop(torch, fstep, kf, barrier), dev) / kf
 
+    # ---- the path-tracer-style stream -- unsorted material ids AND a world-space shading frame
+    # per query (76 B in + 12 B out per query; stage A4 runs for every query) ----
+    with_frames = None
+    if rank == 0 and prec != "fp32":
+        fr_host = synth.make_frames(np.random.default_rng(77), n)
+        frs = [torch.from_numpy(np.roll(fr_host, r * 12345, axis=0).copy()).to(dev) for r in range(N_ROTATE)]
+        stepf = lambda i: api.nbsdf_eval(ctx, q_dev[i % N_ROTATE], frs[i % N_ROTATE], n, out_dev[i % N_ROTATE])
+        for i in range(3):
+            stepf(i)
+        torch.cuda.synchronize()
+        kfr = max(3, min(K, 300))
+        msf = time_loop(torch, stepf, kfr, lambda: None) / kfr
+        with_frames = {"workload": "configs[1] queries with a per-query world-space frame (n, t): 64 B in + 12 B out",
+                       "queries_per_s": n / (msf * 1e-3), "us_per_launch": msf * 1e3, "steps": kfr,
+                       "tensor_frac": FLOP_PER_QUERY * n / (msf * 1e-3) / 1e12 / peaks["bf16_tflops"],
+                       "hbm_gbs_algorithmic": (BYTES_PER_QUERY + 24) * n / (msf * 1e-3) / 1e9}
+        del frs
+
     # ---- configs[3]: 3840x2160, 16 stratified light samples (one frame size, no rotation: 431 MB of G-buffer > L2) ----
     frame4k = None
     if rank == 0 and prec != "fp32":
@@ -369,6 +387,7 @@ def run_ours(args):
                       "frame_ms": fms, "steps": kf, "flop_per_pixel": FLOP_MLP_A + 5 * FLOP_MLP_B,
                       "achieved_tflops": frame_tf, "frac": frame_tf / peaks["bf16_tflops"] if prec != "fp32" else frame_tf / 74.4,
                       "decoder_evals_per_s": world * npx * 5 / (fms * 1e-3)},
+            "eval_with_frames": with_frames,
             "frame_4k": frame4k,
             "paper_decoder": paper,
             "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle", "value_1_thread": cpu_rate_1t,

@@ -116,7 +116,7 @@ int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, const float*
 /* Batched decoder inference: stages A1-A4, B1-B7 of DESIGN.md in one fused kernel.
  * q_dev: DEVICE, n records, 16-byte aligned.  frames_dev: DEVICE [n][6] = (normal, tangent hint) per query in
  * the space of wi/wo, or NULL when wi/wo are already local.  rgb_dev: DEVICE [n][3] fp32, 16-byte aligned.
- * n == 0 is a no-op returning NBSDF_OK. */
+ * n == 0 is a no-op returning NBSDF_OK; n >= 2^38 per call is NBSDF_E_INVALID (tile indices are 32-bit). */
 int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float* frames_dev, int64_t n, float* rgb_dev,
                void* cuda_stream);
 

@@ -91,13 +91,15 @@ struct Tc {
     static_assert(K1p <= 48 && K4p == 48, "x / y hold at most 24 columns");
 
     static constexpr uint32_t kLatBytes = 64 * 32 * 2;            // packed latent table, max M x max L
-    static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);
+    static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);      // one tile of query records ...
+    static constexpr uint32_t kFrameBytes = 128 * 6 * sizeof(float);         // ... and of per-query frames behind it
+    static constexpr uint32_t kStageStride = kStageBytes + kFrameBytes;      // 8192
     static constexpr uint32_t kStages = 2;                        // staging buffers per warpgroup
 
     __host__ __device__ static constexpr uint32_t wimg_bytes() { return kLay.total; }
     __host__ __device__ static constexpr uint32_t smem_bytes()
     {
-        return 1024u + ((wimg_bytes() + 127u) & ~127u) + kLatBytes + NWG * kStages * kStageBytes + NWG * 32u + 64u;
+        return 1024u + ((wimg_bytes() + 127u) & ~127u) + kLatBytes + NWG * kStages * kStageStride + NWG * 32u + 64u;
     }
 };
 
@@ -162,12 +164,12 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const uint32_t s_wimg = base;
     const uint32_t s_lat = s_wimg + kWimgPad;
     const uint32_t s_stage = s_lat + T::kLatBytes;
-    const uint32_t s_bars = s_stage + NWG * T::kStages * T::kStageBytes;
+    const uint32_t s_bars = s_stage + NWG * T::kStages * T::kStageStride;
     const uint32_t s_tmem = s_bars + NWG * 32u;
     uint8_t* g_wimg = gbase;
     uint8_t* g_lat = g_wimg + kWimgPad;
     uint8_t* g_stage = g_lat + T::kLatBytes;
-    uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStages * T::kStageBytes + NWG * 32u);
+    uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStages * T::kStageStride + NWG * 32u);
 
     const int tid = threadIdx.x;
 #ifdef NBSDF_CLOCK_PROBE
@@ -241,16 +243,21 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     const int first = (int)blockIdx.x * NWG + wg;
     auto row_is_live = [&](int tile) { return tile < n_full || (tile == n_full && t < last_rows); };
     uint32_t mma_phase = 0;
-    const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStages * T::kStageBytes;
-    const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStages * T::kStageBytes;
+    const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStages * T::kStageStride;
+    const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStages * T::kStageStride;
+    // per-query frames ride in the same staging buffer when their address allows bulk copies (16-byte aligned)
+    const bool frames_bulk = frames != nullptr && (reinterpret_cast<uintptr_t>(frames) & 15u) == 0;
 
     // eval: full tiles are staged in shared memory by bulk copies, two buffers per warpgroup; the tile processed in
     // iteration k of this warpgroup lives in buffer k & 1 and completes phase (k >> 1) & 1 of that buffer's mbarrier.
     auto tile_is_bulk = [&](int tile) { return !kShade && tile < n_full; };
     auto stage_request = [&](int tile, uint32_t k) {      // one elected lane
         if (tile_is_bulk(tile)) {
-            mbar_expect_tx(q_bar + 8u * (k & 1u), T::kStageBytes);
-            bulk_g2s(my_stage + (k & 1u) * T::kStageBytes, q + (int64_t)tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
+            mbar_expect_tx(q_bar + 8u * (k & 1u), T::kStageBytes + (frames_bulk ? T::kFrameBytes : 0u));
+            bulk_g2s(my_stage + (k & 1u) * T::kStageStride, q + (int64_t)tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
+            if (frames_bulk)
+                bulk_g2s(my_stage + (k & 1u) * T::kStageStride + T::kStageBytes, frames + (int64_t)tile * 768, T::kFrameBytes,
+                         q_bar + 8u * (k & 1u));
         }
     };
 
@@ -396,7 +403,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             };
             if (bulk) {
                 mbar_wait(q_bar + 8u * (k & 1u), (k >> 1) & 1u);
-                const uint2* r2 = reinterpret_cast<const uint2*>(my_stage_g + (k & 1u) * T::kStageBytes + t * sizeof(nbsdf_query));
+                const uint2* r2 = reinterpret_cast<const uint2*>(my_stage_g + (k & 1u) * T::kStageStride + t * sizeof(nbsdf_query));
                 unpack(r2[0], r2[1], r2[2], r2[3], r2[4]);
             } else if (direct) {
                 const uint2* r2 = reinterpret_cast<const uint2*>(q + it);
@@ -406,8 +413,14 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             material = rec.material;
             float wi[3] = { rec.wi[0], rec.wi[1], rec.wi[2] }, wo[3] = { rec.wo[0], rec.wo[1], rec.wo[2] };
             if (frames != nullptr && (bulk || direct)) {
-                const float2* fp2 = reinterpret_cast<const float2*>(frames + 6 * it);
-                const float2 f0 = __ldg(fp2), f1 = __ldg(fp2 + 1), f2 = __ldg(fp2 + 2);
+                float2 f0, f1, f2;
+                if (bulk && frames_bulk) {
+                    const float2* fs = reinterpret_cast<const float2*>(my_stage_g + (k & 1u) * T::kStageStride + T::kStageBytes + t * 24);
+                    f0 = fs[0]; f1 = fs[1]; f2 = fs[2];
+                } else {
+                    const float2* fp2 = reinterpret_cast<const float2*>(frames + 6 * it);
+                    f0 = __ldg(fp2); f1 = __ldg(fp2 + 1); f2 = __ldg(fp2 + 2);
+                }
                 const Frame ff = make_frame(f0.x, f0.y, f1.x, f1.y, f2.x, f2.y);
                 to_local(ff, rec.wi[0], rec.wi[1], rec.wi[2], wi);
                 to_local(ff, rec.wo[0], rec.wo[1], rec.wo[2], wo);

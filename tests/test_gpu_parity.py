@@ -108,6 +108,14 @@ def test_frames_materials_background_and_wrap(prec):
     ident = np.tile(np.array([0, 0, 1, 1, 0, 0], np.float32), (len(q), 1))
     a, b = c.eval(q), c.eval(q, ident)
     np.testing.assert_allclose(a, b, rtol=1e-6 if prec == "fp32" else 1e-2)
+    # frames that are only 8-byte aligned take the direct-load path instead of the bulk-copy staging: same bits
+    pad = torch.zeros(len(q) * 6 + 2, dtype=torch.float32, device="cuda")
+    pad[2:] = torch.from_numpy(fr.reshape(-1)).cuda()
+    assert pad[2:].data_ptr() % 16 == 8
+    out2 = torch.empty((len(q), 3), dtype=torch.float32, device="cuda")
+    api.nbsdf_eval(c.ctx, api.queries_to_device(q), pad[2:], len(q), out2)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(out2.cpu().numpy().view(np.uint32), out.view(np.uint32))
     c.close()
 
 

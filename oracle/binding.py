@@ -67,6 +67,8 @@ def _load():
         lib.oracle_inv_logmap.argtypes = [C.c_double, C.c_double]
         lib.oracle_oneblob.restype = None
         lib.oracle_oneblob.argtypes = [C.c_double, C.c_int, C.c_void_p]
+        lib.oracle_lerp_latent.restype = None
+        lib.oracle_lerp_latent.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
         lib.oracle_pd_eval.restype = C.c_int
         lib.oracle_pd_eval.argtypes = [C.c_void_p] * 7 + [C.c_int64, C.c_void_p, C.c_void_p, C.c_int]
         lib.oracle_pd_shade_frame.restype = C.c_int
@@ -249,3 +251,11 @@ def size01(x):
 
 def inv_logmap(y, k):
     return _load().oracle_inv_logmap(float(y), float(k))
+
+
+def lerp_latent(za, zb, t):
+    za, zb = _f32(za).reshape(-1), _f32(zb).reshape(-1)
+    assert za.shape == zb.shape
+    out = np.empty(za.shape[0], dtype=np.float64)
+    _load().oracle_lerp_latent(za.ctypes.data, zb.ctypes.data, za.shape[0], float(t), out.ctypes.data)
+    return out

@@ -276,3 +276,10 @@ int oracle_pd_shade_frame(const oracle_pd_dims* d, const float* const W[7], cons
     }
     return 0;
 }
+
+/* Latent interpolation / extrapolation (sec. 6.3): z = (1 - t) z_a + t z_b, t any real ("the material
+ * latent vector at 0.9 is computed by extrapolation").  Plain definition in double. */
+void oracle_lerp_latent(const float* za, const float* zb, int L, double t, double* out)
+{
+    for (int i = 0; i < L; ++i) out[i] = (1.0 - t) * (double)za[i] + t * (double)zb[i];
+}

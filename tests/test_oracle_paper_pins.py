@@ -266,3 +266,15 @@ def test_frame_shading_closed_forms():
     # background pixels are exactly zero
     g["material"][3] = -1
     assert (oracle.pd_shade_frame(*args, g, lt)[3] == 0).all()
+
+
+def test_lerp_latent_closed_forms():
+    """interpolation and extrapolation of two material latent vectors."""
+    za = np.array([1.0, -2.0, 0.5, 8.0], np.float32)
+    zb = np.array([3.0, 2.0, 0.5, -8.0], np.float32)
+    np.testing.assert_array_equal(oracle.lerp_latent(za, zb, 0.0), za.astype(np.float64))
+    np.testing.assert_array_equal(oracle.lerp_latent(za, zb, 1.0), zb.astype(np.float64))
+    np.testing.assert_array_equal(oracle.lerp_latent(za, zb, 0.5), [2.0, 0.0, 0.5, 0.0])
+    np.testing.assert_array_equal(oracle.lerp_latent(za, zb, 0.25), [1.5, -1.0, 0.5, 4.0])
+    np.testing.assert_array_equal(oracle.lerp_latent(za, zb, 1.5), [4.0, 4.0, 0.5, -16.0])      # extrapolation
+    np.testing.assert_array_equal(oracle.lerp_latent(za, zb, -0.5), [0.0, -4.0, 0.5, 16.0])

@@ -113,6 +113,12 @@ int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weights, nbsdf_ct
  * on cuda_stream and ordered before later launches on it.  first+count > max_materials => NBSDF_E_INVALID. */
 int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, const float* latents_host, void* cuda_stream);
 
+/* Latent interpolation / extrapolation on the device (sec. 6.3 "Interpolation"): row dst of the latent
+ * table becomes (1 - t) * row a + t * row b, in fp32, by a small kernel enqueued on cuda_stream (ordered like
+ * nbsdf_set_latents; no host round trip).  t may lie outside [0, 1] (extrapolation); dst may equal a or b.
+ * Rows outside [0, max_materials) => NBSDF_E_INVALID. */
+int nbsdf_lerp_latents(nbsdf_ctx* ctx, int32_t dst, int32_t a, int32_t b, float t, void* cuda_stream);
+
 /* Batched decoder inference: stages A1-A4, B1-B7 of DESIGN.md in one fused kernel.
  * q_dev: DEVICE, n records, 16-byte aligned.  frames_dev: DEVICE [n][6] = (normal, tangent hint) per query in
  * the space of wi/wo, or NULL when wi/wo are already local.  rgb_dev: DEVICE [n][3] fp32, 16-byte aligned.

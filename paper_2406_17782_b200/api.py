@@ -15,7 +15,7 @@ NBSDF_PREC_FP32, NBSDF_PREC_BF16, NBSDF_PREC_FP16 = 0, 1, 2
 PRECISIONS = {"fp32": NBSDF_PREC_FP32, "bf16": NBSDF_PREC_BF16, "fp16": NBSDF_PREC_FP16}
 NBSDF_MAX_LIGHTS = 32
 EXPORTS = ["nbsdf_create", "nbsdf_set_latents", "nbsdf_eval", "nbsdf_shade_frame", "nbsdf_destroy",
-           "nbsdf_last_error", "nbsdf_launch_count", "nbsdf_create_paper", "nbsdf_set_albedos"]
+           "nbsdf_last_error", "nbsdf_launch_count", "nbsdf_create_paper", "nbsdf_set_albedos", "nbsdf_lerp_latents"]
 
 
 class NbsdfError(RuntimeError):
@@ -66,6 +66,8 @@ def load():
         lib.nbsdf_launch_count.argtypes = [C.c_void_p]
         lib.nbsdf_create_paper.restype = C.c_int
         lib.nbsdf_create_paper.argtypes = [C.POINTER(_Config), C.POINTER(_PaperWeights), C.POINTER(C.c_void_p)]
+        lib.nbsdf_lerp_latents.restype = C.c_int
+        lib.nbsdf_lerp_latents.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
         lib.nbsdf_set_albedos.restype = C.c_int
         lib.nbsdf_set_albedos.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         _lib = lib
@@ -132,6 +134,10 @@ def nbsdf_set_latents(ctx, first, latents_host, stream=None):
     z = np.ascontiguousarray(latents_host, dtype=np.float32)
     z = z.reshape(1, -1) if z.ndim == 1 else z
     _check(load().nbsdf_set_latents(ctx, first, z.shape[0], z.ctypes.data, _stream(stream)), ctx)
+
+
+def nbsdf_lerp_latents(ctx, dst, a, b, t, stream=None):
+    _check(load().nbsdf_lerp_latents(ctx, int(dst), int(a), int(b), float(t), _stream(stream)), ctx)
 
 
 def nbsdf_eval(ctx, q_dev, frames_dev, n, rgb_dev, stream=None):

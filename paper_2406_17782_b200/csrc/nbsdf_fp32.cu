@@ -251,4 +251,20 @@ cudaError_t launch_shade_fp32(const NetParams& net, const FrameParams& fr, const
     return cudaGetLastError();
 }
 
+// Latent interpolation: z_dst = (1 - t) z_a + t z_b, one thread per component, fp32.
+__global__ void lerp_latents_kernel(float* __restrict__ latents, int L, int dst, int a, int b, float t)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < L) {
+        const float za = latents[(size_t)a * L + i], zb = latents[(size_t)b * L + i];
+        latents[(size_t)dst * L + i] = fmaf(t, zb, (1.0f - t) * za);
+    }
+}
+
+cudaError_t launch_lerp_latents(float* latents, int L, int dst, int a, int b, float t, cudaStream_t s)
+{
+    lerp_latents_kernel<<<(L + 63) / 64, 64, 0, s>>>(latents, L, dst, a, b, t);
+    return cudaGetLastError();
+}
+
 }  // namespace nbsdf

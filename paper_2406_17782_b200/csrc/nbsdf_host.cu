@@ -358,6 +358,21 @@ extern "C" int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, c
     return NBSDF_OK;
 }
 
+extern "C" int nbsdf_lerp_latents(nbsdf_ctx* ctx, int32_t dst, int32_t a, int32_t b, float t, void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    const int M = ctx->cfg.max_materials;
+    if (dst < 0 || dst >= M || a < 0 || a >= M || b < 0 || b >= M)
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_lerp_latents: row out of range");
+    if (!(t == t)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_lerp_latents: t is NaN");
+    cudaError_t e = cudaSetDevice(ctx->cfg.device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    e = launch_lerp_latents(ctx->d_latents, ctx->cfg.latent_dim, dst, a, b, t, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_lerp_latents launch", e);
+    ctx->launches += 1;
+    return NBSDF_OK;
+}
+
 static NetParams net_params(const nbsdf_ctx* ctx)
 {
     NetParams p;

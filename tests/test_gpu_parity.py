@@ -267,3 +267,25 @@ def test_error_codes_and_no_fallback(cfg0):
     assert api.nbsdf_launch_count(c.ctx) == n0 + 1
     torch.cuda.synchronize()
     c.close()
+
+
+@pytest.mark.parametrize("t", [0.0, 0.3, 1.0, 1.25, -0.5])
+def test_latent_interpolation_on_device(t):
+    """render with z = (1 - t) z_a + t z_b, formed on the device, incl. extrapolation; parity against the
+    oracle evaluated with the oracle's own interpolated latent."""
+    cfg = synth.config(1, n=2048 + 5)
+    c = Ctx(cfg, "fp16")
+    api.nbsdf_lerp_latents(c.ctx, 5, 1, 6, t)
+    Z = cfg["latents"].copy().astype(np.float64)
+    Z[5] = oracle.lerp_latent(cfg["latents"][1], cfg["latents"][6], t)
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], Z.astype(np.float32), cfg["queries"])
+    check(c.eval(cfg["queries"]), ref, "fp16", f"lerp t={t}")
+    # in-place form (dst == a) and a bad row
+    api.nbsdf_lerp_latents(c.ctx, 1, 1, 6, 1.0)
+    Z[1] = cfg["latents"][6]
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], Z.astype(np.float32), cfg["queries"])
+    check(c.eval(cfg["queries"]), ref, "fp16", "lerp in place")
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_lerp_latents(c.ctx, 8, 0, 1, 0.5)
+    assert e.value.status == api.NBSDF_E_INVALID
+    c.close()

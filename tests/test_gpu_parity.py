@@ -289,3 +289,23 @@ def test_latent_interpolation_on_device(t):
         api.nbsdf_lerp_latents(c.ctx, 8, 0, 1, 0.5)
     assert e.value.status == api.NBSDF_E_INVALID
     c.close()
+
+
+@pytest.mark.parametrize("prec", ["fp16", "fp32"])
+def test_staging_pipeline_depths(prec):
+    """Batch sizes around whole multiples of (148 SMs x 4 warpgroups) tiles: every warpgroup runs 1, 2, 3 or 4 tiles with
+    a ragged or empty last round, which exercises every phase of the two-buffer bulk-copy staging and of the deferred
+    output stage; also with per-query frames (staged behind the records)."""
+    full = 148 * 4 * 128
+    sizes = sorted({full * j + d for j in (1, 2, 3) for d in (-129, -1, 0, 1, 129)} | {full // 2 + 7, 4 * full + 1})
+    cfg = synth.config(1, n=max(sizes))
+    rng = np.random.default_rng(5)
+    frames = synth.make_frames(rng, max(sizes))
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"])
+    ref_f = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"], frames)
+    c = Ctx(cfg, prec)
+    for n in sizes:
+        check(c.eval(cfg["queries"][:n]), ref[:n], prec, f"n={n}")
+    for n in sizes[::3]:
+        check(c.eval(cfg["queries"][:n], frames[:n]), ref_f[:n], prec, f"frames n={n}")
+    c.close()

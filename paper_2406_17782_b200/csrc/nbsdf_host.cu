@@ -227,10 +227,12 @@ extern "C" int nbsdf_create_paper(const nbsdf_config* cfg, const nbsdf_paper_wei
         if (!weights->W[l] || !weights->b[l]) return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create_paper: NULL weight or bias pointer");
     if (cfg->precision < NBSDF_PREC_FP32 || cfg->precision > NBSDF_PREC_FP16)
         return fail(nullptr, NBSDF_E_INVALID, "nbsdf_create_paper: unknown precision");
-    if (cfg->precision == NBSDF_PREC_FP32 || cfg->latent_dim != kPdLatent || cfg->hidden != 64 || cfg->feat_dim != kFeat ||
+    // bf16 operands are rejected, not served at a private tolerance: the log-mapped specular outputs turn the absolute
+    // error of 8-bit significands through seven layers into 4e-2 relative, outside the 1e-2 bound
+    if (cfg->precision != NBSDF_PREC_FP16 || cfg->latent_dim != kPdLatent || cfg->hidden != 64 || cfg->feat_dim != kFeat ||
         cfg->max_materials < 1 || cfg->max_materials > 64)
         return fail(nullptr, NBSDF_E_UNSUPPORTED,
-                    "nbsdf_create_paper: supported are latent_dim 64, hidden 64, feat_dim 32, 1..64 materials, fp16/bf16 operands");
+                    "nbsdf_create_paper: supported are latent_dim 64, hidden 64, feat_dim 32, 1..64 materials, fp16 operands");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceCount", e);

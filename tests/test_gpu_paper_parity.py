@@ -1,10 +1,10 @@
 """Parity of the paper-structured CUDA decoder (nbsdf_create_paper, through the C ABI) against its fp64 oracle.  -m gpu.
 
-Tolerance: the same metric as the BASELINE.json decoder,
-rel = |gpu - ref| / max(|ref|, 1e-6) per channel.  fp16 operands (the default): north_star's max <= 1e-2 and
-mean <= 2e-3.  bf16 operands: max <= 4e-2, mean <= 4e-3 -- the specular outputs are log-mapped, so an
-ABSOLUTE error d of the raw output o ~ 3 becomes a RELATIVE error d of S = (e^o - 1)/k, and one bf16 rounding of an
-activation of that size is already 2^-9 * 4 = 8e-3; seven layers and the skip connection add up from there.
+Tolerance: the same metric and bounds as the BASELINE.json decoder,
+rel = |gpu - ref| / max(|ref|, 1e-6) per channel, max <= 1e-2 and mean <= 2e-3 (north_star), over all outputs of a case.
+Operands are fp16.  bf16 operands are REJECTED at nbsdf_create_paper (NBSDF_E_UNSUPPORTED): the specular outputs are
+log-mapped, so an ABSOLUTE error d of the raw output o ~ 3 becomes a RELATIVE error d of
+S = (e^o - 1)/k, and 8-bit significands through seven layers measured 4e-2 -- outside the bound, so the mode is not shipped.
 The synthetic network (synth.make_pd_network) keeps the BSDF values positive and O(1), as a BSDF's are.
 """
 import numpy as np
@@ -17,8 +17,8 @@ torch = pytest.importorskip("torch")
 import oracle  # noqa: E402
 from paper_2406_17782_b200 import api, synth  # noqa: E402
 
-PRECS = ["fp16", "bf16"]
-TOL = {"fp16": (1e-2, 2e-3), "bf16": (4e-2, 4e-3)}
+PRECS = ["fp16"]
+TOL = {"fp16": (1e-2, 2e-3)}
 
 
 def check(gpu, ref, what="", prec="fp16"):
@@ -28,7 +28,7 @@ def check(gpu, ref, what="", prec="fp16"):
     assert np.isfinite(gpu).all(), what
     r = np.abs(gpu - ref) / np.maximum(np.abs(ref), 1e-6)
     mx, mean = r.max(axis=0), r.mean(axis=0)
-    assert (mx <= TMAX).all() and ((mean <= TMEAN).all() or len(ref) < 64), f"{what}: max {mx} mean {mean}"
+    assert (mx <= TMAX).all() and (mean <= TMEAN).all(), f"{what}: max {mx} mean {mean}"
     return mx, mean
 
 
@@ -70,11 +70,16 @@ def test_paper_eval_small_and_tile_edges(prec):
     ref = oracle.pd_eval_queries(*_args(cfg), cfg["queries"])
     c = PCtx(cfg, prec)
     check(c.eval(cfg["queries"]), ref, f"paper eval {prec}", prec)
+    outs, refs = [], []
     for n in (0, 1, 127, 128, 129, 1025):
         out = c.eval(cfg["queries"][:n])
         assert out.shape == (n, 3)
-        if n:
-            check(out, ref[:n], f"paper eval n={n} {prec}", prec)
+        if n:                 # max bound per batch, mean bound on the pooled outputs
+            r = np.abs(out - ref[:n]) / np.maximum(np.abs(ref[:n]), 1e-6)
+            assert np.isfinite(out).all() and r.max() <= TOL[prec][0], f"paper eval n={n}"
+            outs.append(out)
+            refs.append(ref[:n])
+    check(np.concatenate(outs), np.concatenate(refs), f"paper eval tile edges pooled {prec}", prec)
     c.close()
 
 
@@ -134,6 +139,24 @@ def test_paper_frame_shading_and_albedo_edit(prec):
     c.close()
 
 
+def test_paper_frame_with_emitter_normals():
+    """Point lights with an emitter normal (E = I max(0, -wi . n_e) / d^2), one of them behind the fabric, one facing
+    away (contributes exactly 0): pd_kernel's light loop against the oracle."""
+    cfg = synth.pd_config("frame", width=333, height=97, seed=31)
+    g = cfg["gbuffer"]
+    lights = cfg["lights"].copy()
+    lights[1]["emit_n"] = (0.0, 0.6, -0.8)
+    lights[3]["emit_n"] = (0.0, 0.0, 1.0)           # above the fabric, facing up: black
+    lights[5]["emit_n"] = (0.28, 0.0, 0.96)         # behind the fabric, facing it
+    ref = oracle.pd_shade_frame(*_args(cfg), g, lights)
+    c = PCtx(cfg, "fp16")
+    out = c.shade(g, lights)
+    check(out, ref, "paper frame, emitter normals")
+    only = c.shade(g, lights[3:4])
+    assert (only == 0).all()
+    c.close()
+
+
 def test_paper_frame_matches_eval_on_expanded_queries():
     """The frame kernel runs the fusion layers once per pixel; nbsdf_eval on the (pixel, light) list does not."""
     cfg = synth.pd_config("frame", width=64, height=40)
@@ -175,10 +198,12 @@ def test_paper_full_size_batch_and_errors():
     mx, mean = check(c.eval(cfg["queries"]), ref, "paper eval 2^20 fp16")
     print("paper eval 2^20 fp16: max rel", mx, "mean rel", mean)
     c.close()
-    # the fp32 CUDA-core variant is not built for this structure; BASELINE.json contexts have no albedo table
-    with pytest.raises(api.NbsdfError) as e:
-        api.nbsdf_create_paper(cfg["weights"], cfg["biases"], 64, 8, "fp32")
-    assert e.value.status == api.NBSDF_E_UNSUPPORTED
+    # the fp32 CUDA-core variant is not built for this structure and bf16 operands cannot meet the tolerance (see the
+    # module docstring): both are rejected, not silently served; BASELINE.json contexts have no albedo table
+    for bad in ("fp32", "bf16"):
+        with pytest.raises(api.NbsdfError) as e:
+            api.nbsdf_create_paper(cfg["weights"], cfg["biases"], 64, 8, bad)
+        assert e.value.status == api.NBSDF_E_UNSUPPORTED
     c0 = synth.config(0)
     ctx = api.nbsdf_create(c0["weights"], c0["biases"], 16, 64, 1, "fp16")
     with pytest.raises(api.NbsdfError) as e:

@@ -28,9 +28,7 @@ def check(gpu, ref, prec, what=""):
     assert np.isfinite(gpu).all(), what
     mx, mean = rel_err(gpu, ref)
     tmax, tmean = TOL[prec]
-    # the mean bound is a batch statistic: on a handful of outputs it degenerates to a second, tighter max bound
-    mean_ok = (mean <= tmean).all() or np.asarray(ref).reshape(-1, 3).shape[0] < 64
-    assert (mx <= tmax).all() and mean_ok, f"{what} {prec}: max {mx} mean {mean}"
+    assert (mx <= tmax).all() and (mean <= tmean).all(), f"{what} {prec}: max {mx} mean {mean}"
     return mx, mean
 
 
@@ -77,15 +75,22 @@ def test_config0_tiny_eval(cfg0, prec):
 
 @pytest.mark.parametrize("prec", PRECS)
 def test_tile_edges_and_empty(cfg0, prec):
+    """Max bound on every batch; the mean bound (a statistic over all outputs of a case) on the
+    outputs of all the batches pooled, so that a one-query batch is not held to the mean bound as a second max bound."""
     c = Ctx(cfg0, prec)
+    outs, refs = [], []
     for n in (0, 1, 127, 128, 129, 4097 - 1024, 513):
         q = synth.make_queries(np.random.default_rng(n), n, 1)
         out = c.eval(q)
         assert out.shape == (n, 3)
         if n:
             ref = oracle.eval_queries(cfg0["weights"], cfg0["biases"], cfg0["latents"], q)
-            check(out, ref, prec, f"n={n}")
+            assert np.isfinite(out).all()
+            assert (rel_err(out, ref)[0] <= TOL[prec][0]).all(), f"n={n}"
+            outs.append(out)
+            refs.append(ref)
     c.close()
+    check(np.concatenate(outs), np.concatenate(refs), prec, "tile edges, pooled")
 
 
 @pytest.mark.parametrize("prec", PRECS)
@@ -218,22 +223,82 @@ def test_config1_full_size(prec):
     print(f"config 1 {prec}: max rel {mx}, mean rel {mean}")
 
 
-@pytest.mark.parametrize("prec", ["fp16"])
-def test_config2_and_3_full_size_sampled(prec):
-    """Full-size frames in bench.py's launch configuration; oracle on a seeded sample of whole rows."""
-    for idx, n_rows in ((2, 48), (3, 24)):
-        cfg = synth.config(idx)
-        g, lights = cfg["gbuffer"], cfg["lights"]
-        c = Ctx(cfg, prec)
-        out = c.shade(g, lights)
-        c.close()
-        assert np.isfinite(out).all() and (out > 0).all()
-        W, Hh = g["width"], g["height"]
-        rows = np.random.default_rng(idx).choice(Hh, n_rows, replace=False)
-        rows = np.concatenate([rows, [0, 63, 64, Hh - 1]])           # include tile edges and the last row
-        for r in rows:
-            ref = oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, lights, first=int(r) * W, count=W)
-            check(out[int(r) * W:(int(r) + 1) * W], ref, prec, f"config {idx} row {r}")
+def tile_edge_subset(W, Hh, seed, n_min):
+    """Pixel indices (sorted, unique) of a documented subset of a W x Hh frame: every whole row and whole column on either
+    side of a 64-px material-tile edge (0, 63, 64, 127, 128, ...) plus the last row and column, plus a seeded uniform
+    sample that brings the total to at least n_min pixels."""
+    edge_r = sorted({r for r in range(Hh) if r % 64 in (0, 63)} | {Hh - 1})
+    edge_c = sorted({c for c in range(W) if c % 64 in (0, 63)} | {W - 1})
+    mask = np.zeros((Hh, W), bool)
+    mask[edge_r, :] = True
+    mask[:, edge_c] = True
+    rest = np.flatnonzero(~mask.reshape(-1))
+    extra = max(0, n_min - int(mask.sum()))
+    pick = np.random.default_rng(seed).choice(rest, extra, replace=False)
+    mask.reshape(-1)[pick] = True
+    return np.flatnonzero(mask.reshape(-1))
+
+
+def gather_pixels(g, idx):
+    sub = {k: np.ascontiguousarray(g[k][idx]) for k in ("pos_fp", "nrm_u", "tan_v", "material")}
+    sub.update(width=len(idx), height=1, cam_pos=g["cam_pos"])
+    return sub
+
+
+@pytest.fixture(scope="module")
+def cfg2_ref():
+    cfg = synth.config(2)
+    return cfg, oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], cfg["gbuffer"], cfg["lights"])
+
+
+@pytest.fixture(scope="module")
+def cfg3_refs():
+    """configs[3] inputs + the oracle on the tile_edge_subset for frame 1 and for frame 2 (latent of material 3 replaced)"""
+    cfg = synth.config(3)
+    g, lights = cfg["gbuffer"], cfg["lights"]
+    assert (g["width"], g["height"]) == (3840, 2160) and len(lights) == 16
+    idx = tile_edge_subset(g["width"], g["height"], 3, 1 << 20)
+    assert len(idx) >= 1 << 20
+    sub = gather_pixels(g, idx)
+    ref1 = oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], sub, lights)
+    Z2 = cfg["latents"].copy()
+    Z2[cfg["edit_material"]] = cfg["edit_latent"]
+    ref2 = oracle.shade_frame(cfg["weights"], cfg["biases"], Z2, sub, lights)
+    return cfg, idx, ref1, ref2
+
+
+@pytest.mark.parametrize("prec", ["fp16", "bf16"])
+def test_config2_full_size(cfg2_ref, prec):
+    """BASELINE.json configs[2] at 1920x1080 in bench.py's launch configuration; EVERY pixel against the oracle."""
+    cfg, ref = cfg2_ref
+    c = Ctx(cfg, prec)
+    out = c.shade(cfg["gbuffer"], cfg["lights"])
+    c.close()
+    mx, mean = check(out, ref, prec, "config 2 full frame")
+    print(f"config 2 {prec}: max rel {mx}, mean rel {mean}")
+
+
+@pytest.mark.parametrize("prec", ["fp16", "bf16"])
+def test_config3_full_size_with_edit(cfg3_refs, prec):
+    """BASELINE.json configs[3] as stated: 3840x2160, 16 light samples; frame 1, set_latents(3, 1, z'), frame 2; BOTH frames
+    against the oracle on the tile_edge_subset (>= 2^20 pixels incl. every 64-px tile-edge row and column -- the full
+    frame would be 2 x 133 M oracle evaluations); every pixel of a material other than 3 is bit-identical between the
+    two GPU frames over the WHOLE 4K frame."""
+    cfg, idx, ref1, ref2 = cfg3_refs
+    g, lights = cfg["gbuffer"], cfg["lights"]
+    c = Ctx(cfg, prec)
+    f1 = c.shade(g, lights)
+    m = cfg["edit_material"]
+    api.nbsdf_set_latents(c.ctx, m, cfg["edit_latent"])
+    f2 = c.shade(g, lights)
+    c.close()
+    check(f1[idx], ref1, prec, "config 3 frame 1")
+    mx, mean = check(f2[idx], ref2, prec, "config 3 frame 2 (after the edit)")
+    print(f"config 3 {prec} frame 2: max rel {mx}, mean rel {mean}, {len(idx)} pixels checked")
+    same = g["material"] != m
+    np.testing.assert_array_equal(f1[same].view(np.uint32), f2[same].view(np.uint32))
+    assert (f1[~same] != f2[~same]).any()
+    assert np.isfinite(f1).all() and np.isfinite(f2).all() and (f1 > 0).all() and (f2 > 0).all()
 
 
 def test_error_codes_and_no_fallback(cfg0):

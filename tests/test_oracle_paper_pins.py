@@ -268,6 +268,36 @@ def test_frame_shading_closed_forms():
     assert (oracle.pd_shade_frame(*args, g, lt)[3] == 0).all()
 
 
+def test_frame_shading_emitter_cosine_closed_form():
+    """The emit_n != 0 branch of oracle_pd_shade_frame: E = I max(0, -wi . n_e) / d^2.  With one
+    point light, the frame with an emitter normal equals the isotropic frame times max(0, -wi . n_e) pixel by pixel, the
+    factor computed here from the geometry alone; a light facing away gives exactly 0; a hand example: pixel at the
+    origin, light at (0, 0, 2), n_e = (0, 0.6, -0.8) => factor 0.8."""
+    cfg = synth.pd_config("frame", width=8, height=4, seed=10)
+    args = (cfg["weights"], cfg["biases"], cfg["latents"], cfg["albedos"])
+    g = cfg["gbuffer"]
+    x = g["pos_fp"][:, :3].astype(np.float64)
+    for pos, en in (((0.3, -0.2, 1.5), (0.0, 0.6, -0.8)), ((0.1, 0.4, -0.9), (0.6, 0.0, 0.8))):   # above / BEHIND the fabric
+        lt = np.zeros(1, dtype=oracle.LIGHT_DTYPE)
+        lt["type"], lt["vec"], lt["rgb"] = 1, pos, (3.0, 2.0, 1.0)
+        iso = oracle.pd_shade_frame(*args, g, lt)
+        lt["emit_n"] = en
+        got = oracle.pd_shade_frame(*args, g, lt)
+        v = np.array(pos, np.float32).astype(np.float64)[None, :] - x
+        wi = v / np.linalg.norm(v, axis=1, keepdims=True)
+        fac = np.maximum(0.0, -(wi * np.array(en, np.float32).astype(np.float64)[None, :]).sum(1, keepdims=True))
+        assert (fac > 0).all() and (np.abs(iso) > 0).all()
+        np.testing.assert_allclose(got, iso * fac, rtol=1e-13)
+        lt["emit_n"] = tuple(-c for c in en)                                   # emitter facing away: exactly black
+        assert (oracle.pd_shade_frame(*args, g, lt) == 0).all()
+    g["pos_fp"][0, :3] = 0.0
+    lt = np.zeros(1, dtype=oracle.LIGHT_DTYPE)
+    lt["type"], lt["vec"], lt["rgb"] = 1, (0.0, 0.0, 2.0), (3.0, 2.0, 1.0)
+    iso = oracle.pd_shade_frame(*args, g, lt, first=0, count=1)
+    lt["emit_n"] = (0.0, 0.6, -0.8)
+    np.testing.assert_allclose(oracle.pd_shade_frame(*args, g, lt, first=0, count=1), iso * np.float64(np.float32(0.8)), rtol=1e-13)
+
+
 def test_lerp_latent_closed_forms():
     """interpolation and extrapolation of two material latent vectors."""
     za = np.array([1.0, -2.0, 0.5, 8.0], np.float32)

@@ -18,9 +18,29 @@ from paper_2406_17782_b200 import api, synth  # noqa: E402
 
 from test_gpu_parity import Ctx, check  # noqa: E402
 
+HS, LS = [32, 64, 128], [8, 16, 32]
+
+# bf16 operands carry 8-bit significands through four hidden layers; at these two points the max bound is exceeded by the
+# ARITHMETIC, not by the kernel: oracle/quant_study.py (numpy fp64 + bf16 rounding of the operands, no GPU code) gives
+# 1.13e-2 at (L=32, H=64) where the kernel measures 1.14e-2, and 0.5-1.2e-2 over five seeds at H = 32.  The bound is NOT
+# loosened: the points are marked as expected failures, listed in DESIGN.md sec. 2.18, and nbsdf.h tells callers that
+# need the bound at every dims to use fp16 operands (the default), which pass everywhere with 8x margin.
+BF16_INHERENT = "bf16 8-bit significands exceed max 1e-2 here (1.07-1.14e-2), reproduced without the GPU by oracle/quant_study.py"
+
+
+def dims_params(kind):
+    known = {"eval": {(32, 64)}, "shade": {(16, 32)}}[kind]
+    out = []
+    for prec in ("fp16", "bf16"):
+        for L in LS:
+            for H in HS:
+                marks = [pytest.mark.xfail(reason=BF16_INHERENT, strict=False)] if prec == "bf16" and (L, H) in known else []
+                out.append(pytest.param(prec, L, H, marks=marks, id=f"{prec}-{L}-{H}"))
+    return out
+
+
 NWG_EVAL = {32: 6, 64: 4, 128: 2}          # warpgroups per CTA (csrc/nbsdf_tc.cu launch_one); an over-estimate is harmless
 NWG_SHADE = {32: 5, 64: 4, 128: 2}
-HS, LS = [32, 64, 128], [8, 16, 32]
 
 
 def num_sms():
@@ -34,9 +54,7 @@ def lights3():
     return lt
 
 
-@pytest.mark.parametrize("H", HS)
-@pytest.mark.parametrize("L", LS)
-@pytest.mark.parametrize("prec", ["fp16", "bf16"])
+@pytest.mark.parametrize("prec,L,H", dims_params("eval"))
 def test_eval_three_rounds_every_dims(prec, L, H):
     n = 3 * num_sms() * NWG_EVAL[H] * 128 + 129
     seed = synth.sweep_seed(1, HS.index(H), LS.index(L))
@@ -55,14 +73,20 @@ def test_eval_three_rounds_every_dims(prec, L, H):
     c.close()
     live = q["material"] >= 0
     assert (out[~live] == 0).all() and (out_f[~live] == 0).all()
+    if prec == "bf16":
+        # sharper than the 1e-2 bound, and independent of it: against the oracle's forward pass with the SAME operand
+        # rounding (oracle/quant_study.py), what remains is fp32 accumulation order and the rare rounding decision that
+        # flips on it -- a staging or phase slip in the bf16 instantiation would be orders of magnitude above this
+        from oracle import quant_study
+        emu = quant_study.forward(cfg, q[live], quant_study.bf16, quant_study.bf16, quant_study.bf16, merged=H <= 64)
+        r = np.abs(out[live] - emu) / np.maximum(np.abs(emu), 1e-6)
+        assert r.max() <= 4e-3 and r.mean() <= 1e-4, f"bf16 kernel vs bf16-rounded oracle: max {r.max()} mean {r.mean()}"
     check(out[live], ref[live], prec, f"eval L={L} H={H} n={n}")
     check(out_f[live], ref_f[live], prec, f"eval+frames L={L} H={H} n={n}")
     np.testing.assert_array_equal(out2.view(np.uint32), out[:n2].view(np.uint32))      # position independence
 
 
-@pytest.mark.parametrize("H", HS)
-@pytest.mark.parametrize("L", LS)
-@pytest.mark.parametrize("prec", ["fp16", "bf16"])
+@pytest.mark.parametrize("prec,L,H", dims_params("shade"))
 def test_shade_three_rounds_every_dims(prec, L, H):
     npx_min = 3 * num_sms() * NWG_SHADE[H] * 128 + 77
     W = 509                                                     # odd width: rows never align with 128-pixel tiles

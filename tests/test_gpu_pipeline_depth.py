@@ -76,11 +76,12 @@ def test_eval_three_rounds_every_dims(prec, L, H):
     if prec == "bf16":
         # sharper than the 1e-2 bound, and independent of it: against the oracle's forward pass with the SAME operand
         # rounding (oracle/quant_study.py), what remains is fp32 accumulation order and the rare rounding decision that
-        # flips on it -- a staging or phase slip in the bf16 instantiation would be orders of magnitude above this
+        # flips on it (one flipped bf16 activation is 2^-8 relative, so the max stays a max; measured mean 3e-7..4e-7) --
+        # a staging or phase slip in the bf16 instantiation would put the MEAN orders of magnitude above this
         from oracle import quant_study
         emu = quant_study.forward(cfg, q[live], quant_study.bf16, quant_study.bf16, quant_study.bf16, merged=H <= 64)
         r = np.abs(out[live] - emu) / np.maximum(np.abs(emu), 1e-6)
-        assert r.max() <= 4e-3 and r.mean() <= 1e-4, f"bf16 kernel vs bf16-rounded oracle: max {r.max()} mean {r.mean()}"
+        assert r.max() <= 1e-2 and r.mean() <= 1e-5, f"bf16 kernel vs bf16-rounded oracle: max {r.max()} mean {r.mean()}"
     check(out[live], ref[live], prec, f"eval L={L} H={H} n={n}")
     check(out_f[live], ref_f[live], prec, f"eval+frames L={L} H={H} n={n}")
     np.testing.assert_array_equal(out2.view(np.uint32), out[:n2].view(np.uint32))      # position independence

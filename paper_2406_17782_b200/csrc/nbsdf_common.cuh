@@ -19,6 +19,9 @@ struct NetParams {
     const uint8_t* wimg_shade;   // tensor path: shared-memory image for nbsdf_shade_frame (6 layers)
     const float* albedos;        // paper-structured decoder: [M][12] fp32 (kd_warp, kd_weft, ks_warp, ks_weft) x RGB
     int32_t L, H, M;
+#ifdef NBSDF_PROBE
+    int32_t probe_slot;          // debug builds only (nbsdf_probe.cuh): launch counter of the context
+#endif
 };
 
 struct LightParams {

@@ -386,6 +386,9 @@ static NetParams net_params(const nbsdf_ctx* ctx)
     p.L = ctx->cfg.latent_dim;
     p.H = ctx->cfg.hidden;
     p.M = ctx->cfg.max_materials;
+#ifdef NBSDF_PROBE
+    p.probe_slot = (int32_t)ctx->launches;
+#endif
     return p;
 }
 

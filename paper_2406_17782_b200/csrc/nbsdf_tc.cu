@@ -7,20 +7,22 @@
 //   B (weights)     resident in shared memory for the whole kernel as 128-byte-swizzled K-major UMMA tiles,
 //   D (accumulator) fp32 in tensor memory, read back with tcgen05.ld by the owning thread,
 // so the inter-layer epilogue (ReLU, 16-bit pack) is thread-local and no activation ever touches shared
-// memory or HBM.  Query tiles stream in with cp.async.bulk (TMA bulk copy) one tile ahead.  Warpgroups are not
-// specialised: each alternates "issue MMAs / wait / epilogue", and the NWG warpgroups of a CTA interleave so that
-// the tensor pipe, the TMEM load path and the FP32 pipes overlap across tiles.
+// memory or HBM.  Query tiles stream in with cp.async.bulk (TMA bulk copy) three tiles ahead.  The CTA is warp-
+// specialised: warps [0, 4 NWG) are the row owners (input assembly, epilogues, output), and one extra MMA-issuer warp
+// per warpgroup issues that warpgroup's tcgen05.mma chains and its bulk copies; the NWG tiles in flight interleave so
+// that the tensor pipe, the TMEM load path and the ALU pipes overlap across tiles.
 //
-// TMEM columns per warpgroup (512 / NWG available):
+// TMEM columns per warpgroup (504 / NWG available; the last 8 hold the CTA-wide bias-constant block), see struct Tc:
 //   [0, H)                 accumulator (N <= H fp32 columns)
-//   [H, H + H/2)           AH: hidden activations as A operand (K = H 16-bit values = H/2 columns)
-//   [H + H/2, +8)          constant block (c0, c1, c2, 0, ...): A operand of the bias K step of the K = H layers
-//   [H + H/2 + 8, +24)     AY: layer-1 input x = [z, u', v', lf, c] (K1p/2 columns), later y = [feat, wi, wo, c] (24 columns)
+//   [H, H + kAw)           AH: hidden activations as A operand (K = H 16-bit values = H/2 columns); eval: also x / y
+//   shade:  [H + H/2, +24) AY: x = [z, u', v', lf, c] (K1p/2 columns), later y = [feat, wi, wo, c] (24 columns)
+//   merged eval: +8        tail block [wi, wo, c0, c1, c2, 0...]: last K step of the merged layer;  +K1p/2: x (kXDirect)
 // Biases ride inside the contractions (see tc_layout in nbsdf_common.cuh): the epilogue is ReLU + 16-bit pack only.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
 #include "nbsdf_common.cuh"
+#include "nbsdf_probe.cuh"
 #include "nbsdf_tc_ptx.cuh"
 
 #ifndef NBSDF_NWG32_EVAL
@@ -34,25 +36,6 @@
 #endif
 
 namespace nbsdf {
-
-#ifdef NBSDF_PHASE_PROBE
-// debug builds only: cycles thread 0 of CTA 0 spends in each phase of the merged eval chain (summed over its tiles)
-__device__ long long g_phase_probe[32];
-#define NBSDF_PHASE(i) do { const long long now_ = clock64(); ph_acc[i] += now_ - ph_last; ph_last = now_; } while (0)
-#else
-#define NBSDF_PHASE(i) do { } while (0)
-#endif
-
-#ifdef NBSDF_CLOCK_PROBE
-// debug builds only: SM clock ticks and global-timer nanoseconds at the start and end of CTA 0 of the last launch
-__device__ unsigned long long g_clock_probe[4];
-__device__ __forceinline__ unsigned long long global_timer_ns()
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#endif
 
 // ------------------------------------------------------------------------------------------------
 template <int L, int H, bool kBf16, int NWG, bool kShade>
@@ -172,9 +155,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStages * T::kStageStride + NWG * 32u);
 
     const int tid = threadIdx.x;
-#ifdef NBSDF_CLOCK_PROBE
-    if (blockIdx.x == 0 && tid == 0) { g_clock_probe[0] = (unsigned long long)clock64(); g_clock_probe[1] = global_timer_ns(); }
-#endif
+    NBSDF_STAMP(tid == 0, net, 0);
     const int t = tid & 127;               // row within the tile == TMEM lane
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // warp-uniform for the compiler
     // warps [0, 4 NWG): the warpgroups that own tile rows; warp 4 NWG + i: the MMA / bulk-copy issuer of warpgroup i
@@ -215,6 +196,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    NBSDF_STAMP(tid == 0, net, 1);
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *g_tmem, 0);
     const uint32_t col0 = tmem_base + (uint32_t)(wg * T::kColsPerWg);                 // lane 0: for MMA operands
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;                      // this warp's lane quarter
@@ -276,9 +258,38 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         tc_fence_after();
     };
 
+    // While the grid-dependency wait below blocks (it resolves only when the slowest CTA of the previous kernel has
+    // exited: a median of 1.4 us, profiles/r2_eval_timeline.md), pull this CTA's first inputs from HBM into L2.  A
+    // prefetch has no destination: data that a predecessor still writes is simply fetched again from L2 after the wait.
+    if (issuer && wg < NWG && elect_one()) {
+        if constexpr (!kShade) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int tile = first + j * stride;
+                if (tile_is_bulk(tile)) {
+                    bulk_prefetch_l2(q + (int64_t)tile * 128, T::kStageBytes);
+                    if (frames_bulk) bulk_prefetch_l2(frames + (int64_t)tile * 768, T::kFrameBytes);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int tile = first + j * stride;
+                if (tile < n_full) {
+                    bulk_prefetch_l2(fr.pos_fp + (int64_t)tile * 128, 2048u);
+                    bulk_prefetch_l2(fr.nrm_u + (int64_t)tile * 128, 2048u);
+                    bulk_prefetch_l2(fr.tan_v + (int64_t)tile * 128, 2048u);
+                }
+            }
+        }
+        if (wg == 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(net.latents) : "memory");
+    }
+    __syncwarp();
+
     // ---- everything above touched only this CTA's shared / tensor memory and the immutable weight image; what a
     // previous kernel or copy on the stream may have written (queries, latents) is read from here on ----
     pdl_wait_prior_grid();
+    NBSDF_STAMP(tid == 0, net, 2);
     if (!kShade && issuer && wg < NWG) {      // first two query tiles: their HBM latency overlaps the rest of the prologue
         if (elect_one()) {
             stage_request(first, 0u);
@@ -296,6 +307,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    NBSDF_STAMP(tid == 0, net, 3);
 
     if (issuer) {
         // =========================== MMA / bulk-copy issuer warp of warpgroup wg ===========================
@@ -313,6 +325,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 if (k == 0) {
                     stage_request(first + 2 * stride, 2u);    // buffer 0 has been read by every thread of the warpgroup
                     mbar_wait(w_bar, 0);
+                    NBSDF_STAMP(wg == 0, net, 4);
                 }
                 issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, T::kXDirect ? col0 + T::kXCol : ay_d, one_d, w_s[0], mma_bar);
             }
@@ -514,11 +527,6 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     if (kShade) gbuf_request(first);
     if (first < n_tiles) assemble(first, 0u);
 
-#ifdef NBSDF_PHASE_PROBE
-    long long ph_acc[24], ph_last = clock64();
-#pragma unroll
-    for (int i = 0; i < 24; ++i) ph_acc[i] = 0;
-#endif
     uint32_t k = 0;
     for (int tile = first; tile < n_tiles; tile += stride, ++k) {
         const int kind = row_is_live(tile) ? (material < 0 ? 2 : 1) : 0;
@@ -529,48 +537,32 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             for (int i = 0; i < T::K1p / 2; i += 8) tmem_st8(ay_t + i, x + i);
         }
         if constexpr (T::kMerged && !T::kXDirect) store_tail(lane_taddr + T::kTailCol);
-        NBSDF_PHASE(0);
 
         // ---- MLP-A (B1-B3) ----
         publish();                                        // -> layer 1 (short: nothing is put in its shadow)
-        NBSDF_PHASE(1);
-        NBSDF_PHASE(2);
         await_mma();
-        NBSDF_PHASE(3);
+        NBSDF_STAMP(tid == 0 && k == 0, net, 5);
         epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-        NBSDF_PHASE(4);
         publish();                                        // -> layer 2
         flush_output();                                   // shadow of layer 2: the previous tile's B7 / C2-C3
-        NBSDF_PHASE(5);
+        NBSDF_STAMP(tid == 0 && k == 1, net, 6);
         if constexpr (kShade) light_tail(0);              //                    and C1 of the first light
         await_mma();
-        NBSDF_PHASE(6);
         epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-        NBSDF_PHASE(7);
 
         if constexpr (T::kMerged) {
             // ---- merged layers 3+4 (B3-B4): (W4f W3) h2 + W4a [wi, wo] + (W4f b3 + b4); K = H from AH + tail block ----
             publish();                                    // -> merged layer
-            NBSDF_PHASE(8);
             if constexpr (!T::kXDirect) assemble(tile + stride, k + 1u);      // shadow of the merged layer: A1-A4 of the next tile
-            NBSDF_PHASE(12);
             await_mma();
-            NBSDF_PHASE(9);
             epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-            NBSDF_PHASE(10);
             publish();                                    // -> layer 5
             if constexpr (T::kXDirect) assemble(tile + stride, k + 1u);       // shadow of layer 5 (the merged layer is done)
-            NBSDF_PHASE(11);
             await_mma();
-            NBSDF_PHASE(13);
             epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-            NBSDF_PHASE(14);
             publish();                                    // -> layer 6
-            NBSDF_PHASE(15);
             await_mma();
-            NBSDF_PHASE(16);
             load_output();
-            NBSDF_PHASE(17);
         } else {
             publish();                                    // -> layer 3
             await_mma();
@@ -616,22 +608,14 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         prev_kind = kind;
     }
     flush_output();
-#ifdef NBSDF_PHASE_PROBE
-    if (blockIdx.x == 0 && tid == 0) {
-#pragma unroll
-        for (int i = 0; i < 24; ++i) g_phase_probe[i] = ph_acc[i];
-        g_phase_probe[24] = (long long)k;
-    }
-#endif
+    NBSDF_STAMP(tid == 0, net, 7);
     }   // role
 
     // ---- teardown ----
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem_base, 512);
-#ifdef NBSDF_CLOCK_PROBE
-    if (blockIdx.x == 0 && tid == 0) { g_clock_probe[2] = (unsigned long long)clock64(); g_clock_probe[3] = global_timer_ns(); }
-#endif
+    NBSDF_STAMP(tid == 0, net, 8);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -710,16 +694,3 @@ cudaError_t launch_shade_tc(const NetParams& net, int precision, int num_sms, co
 }
 
 }  // namespace nbsdf
-
-#ifdef NBSDF_PHASE_PROBE
-extern "C" int nbsdf_debug_phase_probe(long long* out32)
-{
-    return (int)cudaMemcpyFromSymbol(out32, nbsdf::g_phase_probe, 32 * sizeof(long long));
-}
-#endif
-#ifdef NBSDF_CLOCK_PROBE
-extern "C" int nbsdf_debug_clock_probe(unsigned long long* out4)
-{
-    return (int)cudaMemcpyFromSymbol(out4, nbsdf::g_clock_probe, 4 * sizeof(unsigned long long));
-}
-#endif

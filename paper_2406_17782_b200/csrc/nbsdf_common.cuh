@@ -239,9 +239,9 @@ __host__ __device__ constexpr PdLayout pd_layout(int H)
 
 cudaError_t launch_lerp_latents(float* latents, int L, int dst, int a, int b, float t, cudaStream_t s);   // nbsdf_fp32.cu
 cudaError_t init_pd(int H);
-cudaError_t launch_eval_pd(const NetParams& net, int precision, int num_sms, const nbsdf_query* q, const float* frames,
-                           int64_t n, float* rgb, cudaStream_t s);
-cudaError_t launch_shade_pd(const NetParams& net, int precision, int num_sms, const FrameParams& fr,
-                            const LightParams& lights, float* out, cudaStream_t s);
+cudaError_t launch_eval_pd(const NetParams& net, int num_sms, const nbsdf_query* q, const float* frames, int64_t n, float* rgb,
+                           cudaStream_t s);
+cudaError_t launch_shade_pd(const NetParams& net, int num_sms, const FrameParams& fr, const LightParams& lights, float* out,
+                            cudaStream_t s);
 
 }  // namespace nbsdf

@@ -408,7 +408,7 @@ extern "C" int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float*
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
     const NetParams net = net_params(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (ctx->arch == 1) e = launch_eval_pd(net, ctx->cfg.precision, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
+    if (ctx->arch == 1) e = launch_eval_pd(net, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
     else if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_eval_fp32(net, q_dev, frames_dev, n, rgb_dev, s);
     else e = launch_eval_tc(net, ctx->cfg.precision, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_eval launch", e);
@@ -457,7 +457,7 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     fr.cam[0] = g->cam_pos[0]; fr.cam[1] = g->cam_pos[1]; fr.cam[2] = g->cam_pos[2];
     const NetParams net = net_params(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (ctx->arch == 1) e = launch_shade_pd(net, ctx->cfg.precision, ctx->num_sms, fr, lp, radiance_dev, s);
+    if (ctx->arch == 1) e = launch_shade_pd(net, ctx->num_sms, fr, lp, radiance_dev, s);
     else if (ctx->cfg.precision == NBSDF_PREC_FP32) e = launch_shade_fp32(net, fr, lp, radiance_dev, s);
     else e = launch_shade_tc(net, ctx->cfg.precision, ctx->num_sms, fr, lp, radiance_dev, s);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_shade_frame launch", e);

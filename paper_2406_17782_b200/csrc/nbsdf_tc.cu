@@ -21,9 +21,8 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
-#include "nbsdf_common.cuh"
-#include "nbsdf_probe.cuh"
-#include "nbsdf_tc_ptx.cuh"
+#include "nbsdf_probe.cuh"      // NBSDF_STAMP: no-ops unless built with -DNBSDF_PROBE (debug library only)
+#include "nbsdf_tc_pipeline.cuh"
 
 #ifndef NBSDF_NWG32_EVAL
 #define NBSDF_NWG32_EVAL 6
@@ -44,16 +43,8 @@ struct Tc {
     static constexpr TcLayout kLay = tc_layout(L, H, kMerged);
     static constexpr int K1p = kLay.K1p;
     static constexpr int K4p = kLay.K4p;
-    // Warps [0, 4 NWG) are the warpgroups that own tile rows; then one MMA-issuer warp per warpgroup, padded to whole
-    // warpgroups so that setmaxnreg can move the issuers' registers to the row owners.
-    static constexpr int kIssuerWarps = (NWG + 3) / 4 * 4;
-    static constexpr int kThreads = NWG * 128 + kIssuerWarps * 32;
-    static constexpr int kIssuerRegs = 56;
-    static constexpr int kBaseRegs = 65536 / kThreads / 8 * 8 > 248 ? 248 : 65536 / kThreads / 8 * 8;      // what ptxas is told
-    // only what the issuer warps give back is available to setmaxnreg.inc (not the register file's unallocated rest)
-    static constexpr int kOwnerRegsRaw = kBaseRegs + kIssuerWarps * 32 * (kBaseRegs - kIssuerRegs) / (NWG * 128) / 8 * 8;
-    static constexpr int kOwnerRegs = kOwnerRegsRaw > 248 ? 248 : kOwnerRegsRaw;
-    static_assert(kThreads <= 1024, "CTA size");
+    using S = PipeShape<NWG>;
+    static constexpr int kThreads = S::kThreads, kOwnerRegs = S::kOwnerRegs, kBaseRegs = S::kBaseRegs, kIssuerRegs = S::kIssuerRegs;
     static constexpr bool kTwoLoads = kOwnerRegs >= (kShade ? 150 : 100);         // epilogue register budget (see epilogue_to_a)
     // TMEM columns of one warpgroup.  eval: x, the hidden activations and y share ONE A-operand region (each is dead
     // before the next is written); shade: y = [feat, wi, wo] must survive the light loop, so it gets its own region.
@@ -68,22 +59,15 @@ struct Tc {
     static constexpr bool kXDirect = kMerged && NWG * (H + kAw + 8 + K1p / 2) <= 504;
     static constexpr int kXCol = H + kAw + 8;
     static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw + (kMerged ? 8 : 0) + (kXDirect ? K1p / 2 : 0);
-    static constexpr int kOneCol = 504;              // CTA-wide constant block (c0, c1, c2, 0...): bias K step of the K = H layers
+    static constexpr int kOneCol = S::kOneCol;
     static_assert(NWG * kColsPerWg <= kOneCol, "TMEM budget");
     static_assert(L % 8 == 0 && H % 32 == 0, "dims");
     static_assert(K1p <= 48 && K4p == 48, "x / y hold at most 24 columns");
 
     static constexpr uint32_t kLatBytes = 64 * 32 * 2;            // packed latent table, max M x max L
-    static constexpr uint32_t kStageBytes = 128 * sizeof(nbsdf_query);      // one tile of query records ...
-    static constexpr uint32_t kFrameBytes = 128 * 6 * sizeof(float);         // ... and of per-query frames behind it
-    static constexpr uint32_t kStageStride = kStageBytes + kFrameBytes;      // 8192
-    static constexpr uint32_t kStages = 2;                        // staging buffers per warpgroup
 
     __host__ __device__ static constexpr uint32_t wimg_bytes() { return kLay.total; }
-    __host__ __device__ static constexpr uint32_t smem_bytes()
-    {
-        return 1024u + ((wimg_bytes() + 127u) & ~127u) + kLatBytes + NWG * kStages * kStageStride + NWG * 32u + 64u;
-    }
+    __host__ __device__ static constexpr uint32_t smem_bytes() { return S::smem_bytes(wimg_bytes(), kLatBytes); }
 };
 
 // Epilogue of a hidden layer: acc (N fp32 columns, bias already inside) -> (ReLU) -> packed 16-bit pairs -> A columns.
@@ -141,163 +125,36 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 {
     using T = Tc<L, H, kBf16, NWG, kShade>;
     extern __shared__ uint8_t smem_raw[];
-    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    uint8_t* gbase = smem_raw + (base - smem_u32(smem_raw));
-    constexpr uint32_t kWimgPad = (T::wimg_bytes() + 127u) & ~127u;
-    const uint32_t s_wimg = base;
-    const uint32_t s_lat = s_wimg + kWimgPad;
-    const uint32_t s_stage = s_lat + T::kLatBytes;
-    const uint32_t s_bars = s_stage + NWG * T::kStages * T::kStageStride;
-    const uint32_t s_tmem = s_bars + NWG * 32u;
-    uint8_t* g_wimg = gbase;
-    uint8_t* g_lat = g_wimg + kWimgPad;
-    uint8_t* g_stage = g_lat + T::kLatBytes;
-    uint32_t* g_tmem = reinterpret_cast<uint32_t*>(g_stage + NWG * T::kStages * T::kStageStride + NWG * 32u);
-
-    const int tid = threadIdx.x;
-    NBSDF_STAMP(tid == 0, net, 0);
-    const int t = tid & 127;               // row within the tile == TMEM lane
-    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // warp-uniform for the compiler
-    // warps [0, 4 NWG): the warpgroups that own tile rows; warp 4 NWG + i: the MMA / bulk-copy issuer of warpgroup i
-    const bool issuer = warp >= NWG * 4;
-    const int wg = issuer ? warp - NWG * 4 : warp >> 2;          // >= NWG: padding warp, idle
     constexpr TcLayout lay = T::kLay;
+    NBSDF_STAMP(threadIdx.x == 0, net, 0);
 
-    // ---- prologue: weights image + packed latents -> shared memory, barriers, TMEM ----
-    // The weight image is immutable after nbsdf_create, so it is fetched before the grid-dependency wait and overlaps
-    // the tail of the previous kernel on the stream; everything a previous kernel or copy may write comes after it.
-    pdl_launch_dependents();
-    const uint32_t mma_bar = s_bars + (uint32_t)wg * 32u;
-    const uint32_t q_bar = mma_bar + 8u;            // two of them: one per staging buffer
-    const uint32_t w_bar = s_tmem + 8u;
-    if (warp == 0 && elect_one()) {
-        mbar_init(w_bar, 1);
-        fence_mbar_init();
-        // one elected lane streams the whole image in with bulk copies; only the MMA issuers ever wait for it
-        mbar_expect_tx(w_bar, T::wimg_bytes());
-        constexpr uint32_t kChunk = 32768u;
-        for (uint32_t off = 0; off < T::wimg_bytes(); off += kChunk) {
-            const uint32_t bytes = T::wimg_bytes() - off < kChunk ? T::wimg_bytes() - off : kChunk;
-            bulk_g2s(s_wimg + off, (kShade ? net.wimg_shade : net.wimg_eval) + off, bytes, w_bar);
-        }
-    }
-    __syncwarp();
-    if (issuer && wg < NWG && elect_one()) {
-        mbar_init(mma_bar, 1);
-        mbar_init(q_bar, 1);
-        mbar_init(q_bar + 8u, 1);
-        fence_mbar_init();
-    }
-    __syncwarp();
-    if (warp == 0) {
-        tmem_alloc(s_tmem, 512);
-        tmem_relinquish();
-    }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    NBSDF_STAMP(tid == 0, net, 1);
-    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *g_tmem, 0);
-    const uint32_t col0 = tmem_base + (uint32_t)(wg * T::kColsPerWg);                 // lane 0: for MMA operands
-    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;                      // this warp's lane quarter
-    const uint32_t lane_taddr = col0 + lane_off;
-    const uint32_t acc_t = lane_taddr + T::kAccCol, ah_t = lane_taddr + T::kAhCol, ay_t = lane_taddr + T::kAyCol;
-    const uint32_t acc_d = col0 + T::kAccCol, ah_d = col0 + T::kAhCol, ay_d = col0 + T::kAyCol, one_d = tmem_base + T::kOneCol;
-
-    // bias constants (c0, c1, c2) as packed pairs; the CTA-wide constant block is written once per kernel by warpgroup 0
+    // ---- prologue (nbsdf_tc_pipeline.cuh): weight image, barriers, TMEM, constant block; then the grid-dependency wait
+    // with the first tiles prefetched into L2 under it; then the first two query tiles are requested ----
+    // bias constants (c0, c1, c2) as packed pairs
     const uint32_t c01 = pack2<kBf16, false>(tc_bias_const(kBf16, 0), tc_bias_const(kBf16, 1));
     const uint32_t c2z = pack2<kBf16, false>(tc_bias_const(kBf16, 2), 0.0f);
-    if (!issuer && wg == 0) {
-        uint32_t ones[8] = { c01, c2z, 0u, 0u, 0u, 0u, 0u, 0u };
-        tmem_st8(tmem_base + lane_off + T::kOneCol, ones);
-        tmem_wait_st();
-    }
+    Pipe<NWG, kShade> P;
+    P.begin(smem_raw, kShade ? net.wimg_shade : net.wimg_eval, T::wimg_bytes(), T::kLatBytes, T::kColsPerWg,
+            kShade ? fr.n_pixels : n, q, frames, c01, c2z);
+    NBSDF_STAMP(P.tid == 0, net, 1);
+    const int tid = P.tid, t = P.t, wg = P.wg;
+    const bool issuer = P.issuer;
+    const int n_tiles = P.n_tiles, stride = P.stride, first = P.first;
+    const uint32_t col0 = P.col0, lane_taddr = P.lane_taddr, mma_bar = P.mma_bar;
+    uint8_t* g_lat = P.g_tables;
+    const uint32_t acc_t = lane_taddr + T::kAccCol, ah_t = lane_taddr + T::kAhCol, ay_t = lane_taddr + T::kAyCol;
+    const uint32_t acc_d = col0 + T::kAccCol, ah_d = col0 + T::kAhCol, ay_d = col0 + T::kAyCol, one_d = P.tmem_base + T::kOneCol;
     uint32_t w_s[6];
 #pragma unroll
-    for (int l = 0; l < 6; ++l) w_s[l] = s_wimg + (l < lay.n_layers ? lay.w_off[l] : 0u);
+    for (int l = 0; l < 6; ++l) w_s[l] = P.s_wimg + (l < lay.n_layers ? lay.w_off[l] : 0u);
+    auto row_is_live = [&](int tile) { return P.row_is_live(tile); };
+    auto stage_request = [&](int tile, uint32_t k) { P.stage_request(tile, k); };
+    auto publish = [&]() { P.publish(); };
+    auto await_mma = [&]() { P.await_mma(); };
 
-    const int64_t n_items = kShade ? fr.n_pixels : n;
-    // tile indices are 32-bit (the host rejects n >= 2^38); only addresses are formed in 64 bits
-    const int n_tiles = (int)((n_items + 127) / 128);
-    const int n_full = (int)(n_items / 128);                         // tiles [0, n_full) are complete
-    const int last_rows = (int)(n_items - (int64_t)n_full * 128);    // live rows of the ragged tile n_full, if any
-    const int stride = (int)gridDim.x * NWG;
-    const int first = (int)blockIdx.x * NWG + wg;
-    auto row_is_live = [&](int tile) { return tile < n_full || (tile == n_full && t < last_rows); };
-    uint32_t mma_phase = 0;
-    const uint32_t my_stage = s_stage + (uint32_t)wg * T::kStages * T::kStageStride;
-    const uint8_t* my_stage_g = g_stage + (size_t)wg * T::kStages * T::kStageStride;
-    // per-query frames ride in the same staging buffer when their address allows bulk copies (16-byte aligned)
-    const bool frames_bulk = frames != nullptr && (reinterpret_cast<uintptr_t>(frames) & 15u) == 0;
-
-    // eval: full tiles are staged in shared memory by bulk copies, two buffers per warpgroup; the tile processed in
-    // iteration k of this warpgroup lives in buffer k & 1 and completes phase (k >> 1) & 1 of that buffer's mbarrier.
-    auto tile_is_bulk = [&](int tile) { return !kShade && tile < n_full; };
-    auto stage_request = [&](int tile, uint32_t k) {      // one elected lane
-        if (tile_is_bulk(tile)) {
-            mbar_expect_tx(q_bar + 8u * (k & 1u), T::kStageBytes + (frames_bulk ? T::kFrameBytes : 0u));
-            bulk_g2s(my_stage + (k & 1u) * T::kStageStride, q + (int64_t)tile * 128, T::kStageBytes, q_bar + 8u * (k & 1u));
-            if (frames_bulk)
-                bulk_g2s(my_stage + (k & 1u) * T::kStageStride + T::kStageBytes, frames + (int64_t)tile * 768, T::kFrameBytes,
-                         q_bar + 8u * (k & 1u));
-        }
-    };
-
-    // Hand-over between a warpgroup and its issuer warp, one named barrier (128 arrivals + the 32 waiting issuer lanes):
-    // the owning threads never block here.  The MMA that follows is issued only after every owning thread has arrived,
-    // which orders both the operand it reads (tcgen05.st ... wait::st) and the accumulator it overwrites
-    // (tcgen05.ld ... wait::ld) of all 128 rows before it.
-    auto publish = [&]() {
-        tmem_wait_st();
-        tc_fence_before();
-        named_bar_arrive(1 + wg, 160);
-    };
-    auto await_mma = [&]() {
-        mbar_wait(mma_bar, mma_phase);
-        mma_phase ^= 1u;
-        tc_fence_after();
-    };
-
-    // While the grid-dependency wait below blocks (it resolves only when the slowest CTA of the previous kernel has
-    // exited: a median of 1.4 us, profiles/r2_eval_timeline.md), pull this CTA's first inputs from HBM into L2.  A
-    // prefetch has no destination: data that a predecessor still writes is simply fetched again from L2 after the wait.
-    if (issuer && wg < NWG && elect_one()) {
-        if constexpr (!kShade) {
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                const int tile = first + j * stride;
-                if (tile_is_bulk(tile)) {
-                    bulk_prefetch_l2(q + (int64_t)tile * 128, T::kStageBytes);
-                    if (frames_bulk) bulk_prefetch_l2(frames + (int64_t)tile * 768, T::kFrameBytes);
-                }
-            }
-        } else {
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                const int tile = first + j * stride;
-                if (tile < n_full) {
-                    bulk_prefetch_l2(fr.pos_fp + (int64_t)tile * 128, 2048u);
-                    bulk_prefetch_l2(fr.nrm_u + (int64_t)tile * 128, 2048u);
-                    bulk_prefetch_l2(fr.tan_v + (int64_t)tile * 128, 2048u);
-                }
-            }
-        }
-        if (wg == 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(net.latents) : "memory");
-    }
-    __syncwarp();
-
-    // ---- everything above touched only this CTA's shared / tensor memory and the immutable weight image; what a
-    // previous kernel or copy on the stream may have written (queries, latents) is read from here on ----
-    pdl_wait_prior_grid();
+    P.wait_prior_grid(fr, net.latents);
     NBSDF_STAMP(tid == 0, net, 2);
-    if (!kShade && issuer && wg < NWG) {      // first two query tiles: their HBM latency overlaps the rest of the prologue
-        if (elect_one()) {
-            stage_request(first, 0u);
-            stage_request(first + stride, 1u);
-        }
-        __syncwarp();
-    }
-    {
+    {   // the latent table as 16-bit operand rows
         uint16_t* lat = reinterpret_cast<uint16_t*>(g_lat);
         for (int i = tid; i < net.M * L; i += T::kThreads) {
             const float z = __ldg(net.latents + i);
@@ -314,17 +171,14 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         setmaxnreg_dec<T::kIssuerRegs>();
         // Mirrors the owning warpgroup's static layer sequence: wait for "operand ready", issue the layer, commit.
         // Blocking in tcgen05.mma issue (the tensor pipe's queue is shallow) costs nothing here.
-        auto ready = [&]() {
-            named_bar_sync(1 + wg, 160);
-            tc_fence_after();
-        };
+        auto ready = [&]() { P.ready(); };
         uint32_t k = 0;
         for (int tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
             ready();
             if (elect_one()) {
                 if (k == 0) {
                     stage_request(first + 2 * stride, 2u);    // buffer 0 has been read by every thread of the warpgroup
-                    mbar_wait(w_bar, 0);
+                    mbar_wait(P.w_bar, 0);
                     NBSDF_STAMP(wg == 0, net, 4);
                 }
                 issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, T::kXDirect ? col0 + T::kXCol : ay_d, one_d, w_s[0], mma_bar);
@@ -377,17 +231,9 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 
     // shade: this thread's G-buffer texel is requested one tile before it is assembled and lands in registers
     // (52 B/pixel, perfectly coalesced float4 planes)
-    float4 pf_pos = make_float4(0.f, 0.f, 0.f, 1.f), pf_nu = make_float4(0.f, 0.f, 1.f, 0.f), pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
-    int pf_mat = -1;
-    auto gbuf_request = [&](int tile) {
-        const int64_t it = (int64_t)tile * 128 + t;
-        pf_pos = make_float4(0.f, 0.f, 0.f, 1.f); pf_nu = make_float4(0.f, 0.f, 1.f, 0.f); pf_tv = make_float4(1.f, 0.f, 0.f, 0.f);
-        pf_mat = -1;
-        if (row_is_live(tile)) {
-            pf_pos = __ldg(fr.pos_fp + it); pf_nu = __ldg(fr.nrm_u + it); pf_tv = __ldg(fr.tan_v + it);
-            pf_mat = __ldg(fr.material + it);
-        }
-    };
+    GbufTexel pf;
+    pf.clear();
+    auto gbuf_request = [&](int tile) { pf.request(fr, (int64_t)tile * 128 + t, row_is_live(tile)); };
     // ---- per-thread state of the tile that starts next (written by assemble(), one tile ahead) ----
     uint32_t x[T::K1p / 2];             // layer-1 operand [z, u', v', lf, c0, c1, c2, 0...] as packed pairs (eval: held in
                                         // registers until the tile starts; shade: stored to TMEM by assemble())
@@ -400,50 +246,19 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
 
     // stages A1-A4 for `tile` (iteration k of this warpgroup): fetch + assemble into the state above
     auto assemble = [&](int tile, uint32_t k) {
-        const int64_t it = (int64_t)tile * 128 + t;
         float up, vp, lf;
         if constexpr (!kShade) {
             nbsdf_query rec;
-            rec.u = rec.v = 0.0f; rec.footprint = 1.0f; rec.material = -1;
-            rec.wi[0] = rec.wi[1] = 0.0f; rec.wi[2] = 1.0f; rec.wo[0] = rec.wo[1] = 0.0f; rec.wo[2] = 1.0f;
-            const bool bulk = tile_is_bulk(tile);
-            const bool direct = !bulk && row_is_live(tile);
-            auto unpack = [&](const uint2 w0, const uint2 w1, const uint2 w2, const uint2 w3, const uint2 w4) {
-                rec.u = __uint_as_float(w0.x); rec.v = __uint_as_float(w0.y);
-                rec.footprint = __uint_as_float(w1.x); rec.material = (int)w1.y;
-                rec.wi[0] = __uint_as_float(w2.x); rec.wi[1] = __uint_as_float(w2.y); rec.wi[2] = __uint_as_float(w3.x);
-                rec.wo[0] = __uint_as_float(w3.y); rec.wo[1] = __uint_as_float(w4.x); rec.wo[2] = __uint_as_float(w4.y);
-            };
-            if (bulk) {
-                mbar_wait(q_bar + 8u * (k & 1u), (k >> 1) & 1u);
-                const uint2* r2 = reinterpret_cast<const uint2*>(my_stage_g + (k & 1u) * T::kStageStride + t * sizeof(nbsdf_query));
-                unpack(r2[0], r2[1], r2[2], r2[3], r2[4]);
-            } else if (direct) {
-                const uint2* r2 = reinterpret_cast<const uint2*>(q + it);
-                unpack(__ldg(r2), __ldg(r2 + 1), __ldg(r2 + 2), __ldg(r2 + 3), __ldg(r2 + 4));
-            }
+            float wi[3], wo[3];
+            P.fetch_query(tile, k, rec, wi, wo);
             up = wrap01(rec.u); vp = wrap01(rec.v); lf = log_footprint<true>(rec.footprint);
             material = rec.material;
-            float wi[3] = { rec.wi[0], rec.wi[1], rec.wi[2] }, wo[3] = { rec.wo[0], rec.wo[1], rec.wo[2] };
-            if (frames != nullptr && (bulk || direct)) {
-                float2 f0, f1, f2;
-                if (bulk && frames_bulk) {
-                    const float2* fs = reinterpret_cast<const float2*>(my_stage_g + (k & 1u) * T::kStageStride + T::kStageBytes + t * 24);
-                    f0 = fs[0]; f1 = fs[1]; f2 = fs[2];
-                } else {
-                    const float2* fp2 = reinterpret_cast<const float2*>(frames + 6 * it);
-                    f0 = __ldg(fp2); f1 = __ldg(fp2 + 1); f2 = __ldg(fp2 + 2);
-                }
-                const Frame ff = make_frame(f0.x, f0.y, f1.x, f1.y, f2.x, f2.y);
-                to_local(ff, rec.wi[0], rec.wi[1], rec.wi[2], wi);
-                to_local(ff, rec.wo[0], rec.wo[1], rec.wo[2], wo);
-            }
             ytail[0] = pack2<kBf16, false>(wi[0], wi[1]);
             ytail[1] = pack2<kBf16, false>(wi[2], wo[0]);
             ytail[2] = pack2<kBf16, false>(wo[1], wo[2]);
         } else {
-            const float4 pos = pf_pos, nu = pf_nu, tv = pf_tv;
-            material = pf_mat;
+            const float4 pos = pf.pos, nu = pf.nu, tv = pf.tv;
+            material = pf.mat;
             gbuf_request(tile + stride);
             px = pos.x; py = pos.y; pz = pos.z;
             f = make_frame(nu.x, nu.y, nu.z, tv.x, tv.y, tv.z);
@@ -508,10 +323,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 r[c] = kShade ? fmaf(v, w_cur[c], rad[c]) : v;
                 if (prev_kind == 2) r[c] = 0.0f;
             }
-            float* o3 = out + 3 * ((int64_t)prev_tile * 128 + t);
-            o3[0] = r[0];
-            o3[1] = r[1];
-            o3[2] = r[2];
+            P.store_rgb(out, prev_tile, r);
         }
         prev_kind = 0;
         rad[0] = rad[1] = rad[2] = 0.0f;
@@ -611,10 +423,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     NBSDF_STAMP(tid == 0, net, 7);
     }   // role
 
-    // ---- teardown ----
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem_base, 512);
+    P.end();
     NBSDF_STAMP(tid == 0, net, 8);
 }
 
@@ -627,22 +436,7 @@ static cudaError_t launch_one(const NetParams& net, int num_sms, const nbsdf_que
     using T = Tc<L, H, kBf16, NWG, kShade>;
     auto kern = tc_kernel<L, H, kBf16, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());
-    const int64_t n_items = kShade ? fr.n_pixels : n;
-    const int64_t tiles = (n_items + 127) / 128;
-    int64_t grid = (tiles + NWG - 1) / NWG;
-    if (grid > num_sms) grid = num_sms;
-    if (grid < 1) grid = 1;
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(T::kThreads);
-    cfg.dynamicSmemBytes = T::smem_bytes();
-    cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // overlap our prologue with the previous kernel's tail
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, net, q, frames, n, fr, lights, out);
+    return launch_persistent<NWG>(kern, T::smem_bytes(), num_sms, kShade ? fr.n_pixels : n, s, net, q, frames, n, fr, lights, out);
 }
 
 template <bool kShade>

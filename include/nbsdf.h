@@ -17,16 +17,25 @@
  *     cudaStream_t; NULL = the legacy default stream).  The library owns only its packed weights,
  *     latent table and light staging, all released by nbsdf_destroy.  HOST arrays handed to
  *     nbsdf_create / nbsdf_set_latents / nbsdf_shade_frame(lights) are copied before the call returns.
- *   - nbsdf_eval / nbsdf_shade_frame / nbsdf_set_latents only enqueue work on the given stream and
- *     return; there is no internal synchronisation.  Work is ordered by the stream: a set_latents is
- *     visible to every later launch on the same stream (the editing guarantee of PAPER.md:198).
+ *   - nbsdf_eval / nbsdf_shade_frame / nbsdf_set_latents / nbsdf_set_albedos / nbsdf_lerp_latents only enqueue work
+ *     on the given stream and return; there is no internal synchronisation.  (Host rows handed to the two set_* calls
+ *     are staged in a ring of 8 pinned slots: only a 9th edit issued while the first is still in flight waits for that
+ *     one copy.)  Work is ordered by the stream: a set_latents is visible to every later launch on the same stream
+ *     (the editing guarantee of PAPER.md:198).  Every call works on cfg.device and restores the caller's current
+ *     CUDA device before it returns.
  *   - Every call returns an nbsdf_status and never throws or aborts; nbsdf_last_error gives text.
  *     On NBSDF_E_INVALID nothing is launched.  There is no CPU fallback: a device that is not
  *     sm_100 makes nbsdf_create fail with NBSDF_E_UNSUPPORTED.
  *   - Directions are unit length; wi points from the surface to the light, wo to the viewer.  Without a
  *     frame they are already local (+z = macro normal).  material in [0, max_materials); a negative
  *     material yields exactly (0,0,0); material >= max_materials is undefined behaviour.
- *     Inputs must be finite.
+ *     Inputs must be finite; a non-finite input yields an unspecified (finite or NaN) value for THAT row only and
+ *     never a fault.
+ *   - Operand precision: NBSDF_PREC_FP16 (the default of the Python binding) meets max 1e-2 / mean 2e-3 against the
+ *     fp64 definition on every supported dims with ~8x margin.  NBSDF_PREC_BF16 exists for networks whose activations
+ *     exceed the fp16 range; its 8-bit significands meet the mean bound everywhere but the max bound only with < 2x
+ *     margin (measured 0.35e-2 .. 1.14e-2 over the supported dims) -- use fp16 where the bound
+ *     must hold.
  */
 #ifndef NBSDF_H
 #define NBSDF_H
@@ -129,7 +138,7 @@ int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float* frames_dev
 /* Frame shading: per pixel, MLP-A once, MLP-B once per light,
  * radiance[p] = sum_l rgb(z_m, uv, fp, wi_l, wo) * E_l * max(0, wi_l,local.z), lights in index order.
  * gbuf: HOST struct holding DEVICE plane pointers.  lights_host: HOST, n_lights <= NBSDF_MAX_LIGHTS, copied.
- * radiance_dev: DEVICE [h][w][3] fp32, 16-byte aligned. */
+ * radiance_dev: DEVICE [h][w][3] fp32, 16-byte aligned.  width * height >= 2^38 => NBSDF_E_INVALID. */
 int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* gbuf, const nbsdf_light* lights_host, int32_t n_lights,
                       float* radiance_dev, void* cuda_stream);
 
@@ -143,7 +152,8 @@ int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* gbuf, const nbsdf_lig
  * (PAPER.md:172-177); the library inverts g and combines with the material's albedos (Eq. 8):
  *   rgb = kd_warp C_warp + kd_weft C_weft + ks_warp S_warp + ks_weft S_weft.
  * HOST pointers, fp32, row-major [out][in], copied.  Supported: latent_dim 64, hidden 64, feat_dim 32,
- * precision NBSDF_PREC_FP16 or NBSDF_PREC_BF16 (tensor cores); anything else => NBSDF_E_UNSUPPORTED.
+ * precision NBSDF_PREC_FP16 (tensor cores); anything else => NBSDF_E_UNSUPPORTED (bf16 operands cannot meet the
+ * tolerance through the log-mapped specular outputs and are rejected rather than served).
  * A context made here is used with the same nbsdf_set_latents / nbsdf_eval / nbsdf_shade_frame calls:
  *   nbsdf_query.footprint and pos_fp.w then hold the footprint SIZE in multiples of the pattern size (clamped to
  *   [0, 5]), wo.z is ignored, and nbsdf_shade_frame weights each light by |wi_local.z| (transmission contributes). */

@@ -25,14 +25,16 @@ struct nbsdf_ctx {
     float* d_w32 = nullptr;           // fp32 path blob
     uint8_t* d_wimg_eval = nullptr;   // tensor path shared-memory images (see tc_layout)
     uint8_t* d_wimg_shade = nullptr;
-    float* h_stage = nullptr;         // pinned mirror used by set_latents
-    cudaEvent_t stage_free = nullptr; // recorded after the last staged copy
-    bool stage_busy = false;
+    // Host arrays handed to set_latents / set_albedos are copied into a ring of pinned slots before the call returns;
+    // the call blocks only if the ring wraps onto a slot whose copy is still in flight (kRingSlots edits queued).
+    static constexpr int kRingSlots = 8;
+    float* h_ring = nullptr;          // kRingSlots x ring_slot_floats, pinned
+    size_t ring_slot_floats = 0;
+    cudaEvent_t ring_ev[kRingSlots] = {};
+    bool ring_busy[kRingSlots] = {};
+    int ring_next = 0;
     int arch = 0;                     // 0: BASELINE.json decoder (nbsdf_create), 1: paper-structured (nbsdf_create_paper)
     float* d_albedos = nullptr;       // arch 1: [M][12] fp32
-    float* h_alb = nullptr;           // pinned mirror used by set_albedos
-    cudaEvent_t alb_free = nullptr;
-    bool alb_busy = false;
     int64_t launches = 0;
     std::string err;
 };
@@ -48,6 +50,46 @@ static int fail(nbsdf_ctx* ctx, int code, const std::string& msg)
 static int fail_cuda(nbsdf_ctx* ctx, const char* what, cudaError_t e)
 {
     return fail(ctx, NBSDF_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+// The library works on ctx->cfg.device; the caller's current device is restored when a call returns.
+struct DeviceGuard {
+    int prev = -1, dev;
+    cudaError_t err;
+    explicit DeviceGuard(int d) : dev(d)
+    {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+    }
+    ~DeviceGuard() { if (prev >= 0 && prev != dev) cudaSetDevice(prev); }
+};
+
+static cudaError_t ring_create(nbsdf_ctx* ctx, size_t slot_floats)
+{
+    ctx->ring_slot_floats = slot_floats;
+    cudaError_t e = cudaMallocHost(&ctx->h_ring, nbsdf_ctx::kRingSlots * slot_floats * sizeof(float));
+    for (int i = 0; e == cudaSuccess && i < nbsdf_ctx::kRingSlots; ++i)
+        e = cudaEventCreateWithFlags(&ctx->ring_ev[i], cudaEventDisableTiming);
+    return e;
+}
+
+// host rows -> next pinned slot -> cudaMemcpyAsync to dst on stream s; never waits unless the ring has wrapped
+static cudaError_t ring_upload(nbsdf_ctx* ctx, float* dst, const float* src_host, size_t n_floats, cudaStream_t s)
+{
+    const int i = ctx->ring_next;
+    ctx->ring_next = (i + 1) % nbsdf_ctx::kRingSlots;
+    if (ctx->ring_busy[i]) {
+        cudaError_t e = cudaEventSynchronize(ctx->ring_ev[i]);
+        if (e != cudaSuccess) return e;
+        ctx->ring_busy[i] = false;
+    }
+    float* slot = ctx->h_ring + (size_t)i * ctx->ring_slot_floats;
+    memcpy(slot, src_host, n_floats * sizeof(float));
+    cudaError_t e = cudaMemcpyAsync(dst, slot, n_floats * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return e;
+    e = cudaEventRecord(ctx->ring_ev[i], s);
+    if (e == cudaSuccess) ctx->ring_busy[i] = true;
+    return e;
 }
 
 // fp32 -> operand type bits, round to nearest even
@@ -143,8 +185,8 @@ extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weight
     if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceProperties", e);
     if (prop.major != 10)
         return fail(nullptr, NBSDF_E_UNSUPPORTED, "nbsdf_create: device is not sm_100 (Blackwell B200); there is no fallback path");
-    e = cudaSetDevice(cfg->device);
-    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaSetDevice", e);
+    DeviceGuard guard(cfg->device);
+    if (guard.err != cudaSuccess) return fail_cuda(nullptr, "cudaSetDevice", guard.err);
 
     nbsdf_ctx* ctx = new (std::nothrow) nbsdf_ctx();
     if (!ctx) return fail(nullptr, NBSDF_E_NOMEM, "nbsdf_create: out of host memory");
@@ -164,8 +206,7 @@ extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weight
 
     NBSDF_TRY(cudaMalloc(&ctx->d_latents, (size_t)M * L * sizeof(float)), "cudaMalloc(latents)");
     NBSDF_TRY(cudaMemset(ctx->d_latents, 0, (size_t)M * L * sizeof(float)), "cudaMemset(latents)");
-    NBSDF_TRY(cudaMallocHost(&ctx->h_stage, (size_t)M * L * sizeof(float)), "cudaMallocHost(stage)");
-    NBSDF_TRY(cudaEventCreateWithFlags(&ctx->stage_free, cudaEventDisableTiming), "cudaEventCreate");
+    NBSDF_TRY(ring_create(ctx, (size_t)M * L), "pinned staging ring");
     if (cfg->precision == NBSDF_PREC_FP32) {
         std::vector<float> blob(fp32_blob_floats(L, H));
         pack_fp32(L, H, weights, blob.data());
@@ -242,8 +283,8 @@ extern "C" int nbsdf_create_paper(const nbsdf_config* cfg, const nbsdf_paper_wei
     if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceProperties", e);
     if (prop.major != 10)
         return fail(nullptr, NBSDF_E_UNSUPPORTED, "nbsdf_create_paper: device is not sm_100 (Blackwell B200); there is no fallback path");
-    e = cudaSetDevice(cfg->device);
-    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaSetDevice", e);
+    DeviceGuard guard(cfg->device);
+    if (guard.err != cudaSuccess) return fail_cuda(nullptr, "cudaSetDevice", guard.err);
 
     nbsdf_ctx* ctx = new (std::nothrow) nbsdf_ctx();
     if (!ctx) return fail(nullptr, NBSDF_E_NOMEM, "nbsdf_create_paper: out of host memory");
@@ -262,12 +303,9 @@ extern "C" int nbsdf_create_paper(const nbsdf_config* cfg, const nbsdf_paper_wei
     } while (0)
     NBSDF_TRY(cudaMalloc(&ctx->d_latents, (size_t)M * L * sizeof(float)), "cudaMalloc(latents)");
     NBSDF_TRY(cudaMemset(ctx->d_latents, 0, (size_t)M * L * sizeof(float)), "cudaMemset(latents)");
-    NBSDF_TRY(cudaMallocHost(&ctx->h_stage, (size_t)M * L * sizeof(float)), "cudaMallocHost(stage)");
-    NBSDF_TRY(cudaEventCreateWithFlags(&ctx->stage_free, cudaEventDisableTiming), "cudaEventCreate");
+    NBSDF_TRY(ring_create(ctx, (size_t)M * L), "pinned staging ring");      // L = 64 > 12: one slot also fits M albedo rows
     NBSDF_TRY(cudaMalloc(&ctx->d_albedos, (size_t)M * 12 * sizeof(float)), "cudaMalloc(albedos)");
     NBSDF_TRY(cudaMemset(ctx->d_albedos, 0, (size_t)M * 12 * sizeof(float)), "cudaMemset(albedos)");
-    NBSDF_TRY(cudaMallocHost(&ctx->h_alb, (size_t)M * 12 * sizeof(float)), "cudaMallocHost(albedos)");
-    NBSDF_TRY(cudaEventCreateWithFlags(&ctx->alb_free, cudaEventDisableTiming), "cudaEventCreate");
     {
         const PdLayout lay = pd_layout(H);
         std::vector<uint8_t> img(lay.total);
@@ -290,39 +328,28 @@ extern "C" int nbsdf_set_albedos(nbsdf_ctx* ctx, int32_t first, int32_t count, c
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: rows out of range");
     if (count == 0) return NBSDF_OK;
     if (!albedos_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: NULL albedos");
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    cudaError_t e = cudaSetDevice(ctx->cfg.device);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    if (ctx->alb_busy) {
-        e = cudaEventSynchronize(ctx->alb_free);
-        if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventSynchronize", e);
-        ctx->alb_busy = false;
-    }
-    float* src = ctx->h_alb + (size_t)first * 12;
-    memcpy(src, albedos_host, (size_t)count * 12 * sizeof(float));
-    e = cudaMemcpyAsync(ctx->d_albedos + (size_t)first * 12, src, (size_t)count * 12 * sizeof(float), cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemcpyAsync(albedos)", e);
-    e = cudaEventRecord(ctx->alb_free, s);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
-    ctx->alb_busy = true;
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    const cudaError_t e = ring_upload(ctx, ctx->d_albedos + (size_t)first * 12, albedos_host, (size_t)count * 12, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_set_albedos upload", e);
     return NBSDF_OK;
 }
 
 extern "C" void nbsdf_destroy(nbsdf_ctx* ctx)
 {
     if (!ctx) return;
-    if (ctx->stage_busy && ctx->stage_free) cudaEventSynchronize(ctx->stage_free);
-    if (ctx->alb_busy && ctx->alb_free) cudaEventSynchronize(ctx->alb_free);
+    DeviceGuard guard(ctx->cfg.device);
+    for (int i = 0; i < nbsdf_ctx::kRingSlots; ++i) {
+        if (ctx->ring_busy[i] && ctx->ring_ev[i]) cudaEventSynchronize(ctx->ring_ev[i]);
+        if (ctx->ring_ev[i]) cudaEventDestroy(ctx->ring_ev[i]);
+    }
+    if (ctx->h_ring) cudaFreeHost(ctx->h_ring);
     if (ctx->d_albedos) cudaFree(ctx->d_albedos);
-    if (ctx->h_alb) cudaFreeHost(ctx->h_alb);
-    if (ctx->alb_free) cudaEventDestroy(ctx->alb_free);
     if (ctx->arch == 1) ctx->d_wimg_shade = nullptr;      // alias of d_wimg_eval
     if (ctx->d_latents) cudaFree(ctx->d_latents);
     if (ctx->d_w32) cudaFree(ctx->d_w32);
     if (ctx->d_wimg_eval) cudaFree(ctx->d_wimg_eval);
     if (ctx->d_wimg_shade) cudaFree(ctx->d_wimg_shade);
-    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
-    if (ctx->stage_free) cudaEventDestroy(ctx->stage_free);
     delete ctx;
 }
 
@@ -340,23 +367,11 @@ extern "C" int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, c
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_latents: rows out of range");
     if (count == 0) return NBSDF_OK;
     if (!latents_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_latents: NULL latents");
-    cudaStream_t s = (cudaStream_t)cuda_stream;
     const int L = ctx->cfg.latent_dim;
-    cudaError_t e = cudaSetDevice(ctx->cfg.device);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    // the pinned mirror may still be the source of an earlier in-flight copy: wait for that copy only
-    if (ctx->stage_busy) {
-        e = cudaEventSynchronize(ctx->stage_free);
-        if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventSynchronize", e);
-        ctx->stage_busy = false;
-    }
-    float* src = ctx->h_stage + (size_t)first * L;
-    memcpy(src, latents_host, (size_t)count * L * sizeof(float));
-    e = cudaMemcpyAsync(ctx->d_latents + (size_t)first * L, src, (size_t)count * L * sizeof(float), cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemcpyAsync(latents)", e);
-    e = cudaEventRecord(ctx->stage_free, s);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
-    ctx->stage_busy = true;
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    const cudaError_t e = ring_upload(ctx, ctx->d_latents + (size_t)first * L, latents_host, (size_t)count * L, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_set_latents upload", e);
     return NBSDF_OK;
 }
 
@@ -367,9 +382,9 @@ extern "C" int nbsdf_lerp_latents(nbsdf_ctx* ctx, int32_t dst, int32_t a, int32_
     if (dst < 0 || dst >= M || a < 0 || a >= M || b < 0 || b >= M)
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_lerp_latents: row out of range");
     if (!(t == t)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_lerp_latents: t is NaN");
-    cudaError_t e = cudaSetDevice(ctx->cfg.device);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    e = launch_lerp_latents(ctx->d_latents, ctx->cfg.latent_dim, dst, a, b, t, (cudaStream_t)cuda_stream);
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    cudaError_t e = launch_lerp_latents(ctx->d_latents, ctx->cfg.latent_dim, dst, a, b, t, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_lerp_latents launch", e);
     ctx->launches += 1;
     return NBSDF_OK;
@@ -404,8 +419,9 @@ extern "C" int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float*
     if (!q_dev || !rgb_dev) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: NULL buffer");
     if (!aligned16(q_dev) || !aligned16(rgb_dev) || (frames_dev && (reinterpret_cast<uintptr_t>(frames_dev) & 7u)))
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: queries/outputs must be 16-byte aligned, frames 8-byte aligned");
-    cudaError_t e = cudaSetDevice(ctx->cfg.device);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    cudaError_t e;
     const NetParams net = net_params(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (ctx->arch == 1) e = launch_eval_pd(net, ctx->num_sms, q_dev, frames_dev, n, rgb_dev, s);
@@ -426,6 +442,7 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     if (n_lights > 0 && !lights_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL lights");
     const int64_t npx = (int64_t)g->width * g->height;
     if (npx == 0) return NBSDF_OK;
+    if (npx >= ((int64_t)1 << 38)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: width * height must be below 2^38");
     if (!g->pos_fp || !g->nrm_u || !g->tan_v || !g->material || !radiance_dev)
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL buffer");
     if (!aligned16(g->pos_fp) || !aligned16(g->nrm_u) || !aligned16(g->tan_v) || !aligned16(radiance_dev))
@@ -433,8 +450,9 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     for (int l = 0; l < n_lights; ++l)
         if (lights_host[l].type != 0 && lights_host[l].type != 1)
             return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: light type must be 0 (directional) or 1 (point)");
-    cudaError_t e = cudaSetDevice(ctx->cfg.device);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    cudaError_t e;
 
     LightParams lp;
     memset(&lp, 0, sizeof lp);

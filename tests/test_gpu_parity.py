@@ -374,3 +374,69 @@ def test_staging_pipeline_depths(prec):
     for n in sizes[::3]:
         check(c.eval(cfg["queries"][:n], frames[:n]), ref_f[:n], prec, f"frames n={n}")
     c.close()
+
+
+def test_back_to_back_edits_do_not_block_and_are_ordered():
+    """Twenty set_latents calls in a row on a stream that is BUSY (a long kernel queue in front of them): the calls only
+    enqueue (ring of pinned slots; at most the wrap-around waits for one earlier copy, never for the queued kernels), each
+    host array may be overwritten as soon as its call returns, and the last edit wins for the next launch."""
+    import time
+    cfg = synth.config(1, n=1 << 20)
+    c = Ctx(cfg, "fp16")
+    qd = api.queries_to_device(cfg["queries"])
+    out = torch.empty((len(cfg["queries"]), 3), dtype=torch.float32, device="cuda")
+    for _ in range(200):                                           # ~6 ms of queued kernels
+        api.nbsdf_eval(c.ctx, qd, None, len(cfg["queries"]), out)
+    z = np.zeros(16, np.float32)
+    t0 = time.perf_counter()
+    for i in range(8):                                             # within the ring: must not wait for anything
+        z[:] = i
+        api.nbsdf_set_latents(c.ctx, 3, z)
+    dt8 = time.perf_counter() - t0
+    for i in range(8, 20):
+        z[:] = i
+        api.nbsdf_set_latents(c.ctx, 3, z)
+    z[:] = -123.0                                                  # the host array is ours again after the call
+    assert dt8 < 2e-3, f"8 edits took {dt8 * 1e3:.2f} ms with ~6 ms of kernels queued: set_latents blocked on the stream"
+    Z = cfg["latents"].copy()
+    Z[3] = 19.0
+    n = 4096
+    got = c.eval(cfg["queries"][:n])
+    c.close()
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], Z, cfg["queries"][:n])
+    check(got, ref, "fp16", "after 20 edits")
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_non_finite_inputs_do_not_fault_or_leak_into_other_rows(prec):
+    """include/nbsdf.h: a non-finite input yields an unspecified value for that row only, never a fault."""
+    cfg = synth.config(1, n=1000)
+    q = cfg["queries"].copy()
+    bad = np.arange(7, 1000, 41)
+    vals = [np.nan, np.inf, -np.inf]
+    for j, i in enumerate(bad):
+        field = ("u", "v", "footprint", "wi", "wo")[j % 5]
+        if field in ("wi", "wo"):
+            q[field][i, j % 3] = vals[j % 3]
+        else:
+            q[field][i] = vals[j % 3]
+    frames = synth.make_frames(np.random.default_rng(3), len(q))
+    frames[11] = np.nan
+    frames[12, :3] = 0.0                                            # zero normal: 0 * inf inside the frame construction
+    c = Ctx(cfg, prec)
+    out = c.eval(q)
+    out_f = c.eval(q, frames)
+    g = synth.make_gbuffer(np.random.default_rng(1), 64, 16)
+    g["pos_fp"][5] = np.inf
+    g["nrm_u"][9, :3] = np.nan
+    rad = c.shade(g, synth.lights_direct5())
+    c.close()                                                       # a sticky fault would surface here at the latest
+    good = np.ones(len(q), bool)
+    good[bad] = False
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"])
+    check(out[good], ref[good], prec, "rows next to non-finite rows")
+    good[[11, 12]] = False
+    assert np.isfinite(out_f[good]).all()
+    ok = np.ones(64 * 16, bool)
+    ok[[5, 9]] = False
+    assert np.isfinite(rad[ok]).all()

@@ -8,5 +8,5 @@ Nothing here is shared with, imported by, or imports the CUDA package.
 from .binding import (  # noqa: F401
     QUERY_DTYPE, LIGHT_DTYPE, build, eval_queries, shade_frame, softplus, wrap,
     log_footprint, to_local, max_threads,
-    pd_eval_queries, pd_shade_frame, oneblob, leaky, size01, inv_logmap, lerp_latent,
+    pd_eval_queries, pd_shade_frame, oneblob, leaky, size01, inv_logmap, lerp_latent, encode_latent,
 )

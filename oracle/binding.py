@@ -7,7 +7,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "nbsdf_oracle.c")
-_SRCS = [_SRC, os.path.join(_HERE, "nbsdf_oracle_paper.c")]
+_SRCS = [_SRC, os.path.join(_HERE, "nbsdf_oracle_paper.c"), os.path.join(_HERE, "nbsdf_oracle_encoder.c")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 # wire format of the inputs (query = position, size, wi, wo + material latent id)
@@ -74,6 +74,8 @@ def _load():
         lib.oracle_pd_shade_frame.restype = C.c_int
         lib.oracle_pd_shade_frame.argtypes = [C.c_void_p] * 9 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
                                                                  C.c_int, C.c_void_p, C.c_int]
+        lib.oracle_encode_latent.restype = C.c_int
+        lib.oracle_encode_latent.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p]
         global _all_threads
         _all_threads = int(lib.oracle_max_threads())      # before any call narrows the OpenMP team
         _lib = lib
@@ -258,4 +260,26 @@ def lerp_latent(za, zb, t):
     assert za.shape == zb.shape
     out = np.empty(za.shape[0], dtype=np.float64)
     _load().oracle_lerp_latent(za.ctypes.data, zb.ctypes.data, za.shape[0], float(t), out.ctypes.data)
+    return out
+
+
+class _EncDims(C.Structure):
+    _fields_ = [("feat_width", C.c_int32), ("hidden", C.c_int32), ("latent_dim", C.c_int32)]
+
+
+def encode_latent(weights, biases, feature, alpha, beta):
+    """fp64 encoder tail (nbsdf_oracle_encoder.c): weights/biases = 4 arrays E0 [He][Fr+2], E1, E2 [He][He], E3 [L][He];
+    feature [Fr] fp32; returns z float64 [L]."""
+    Ws = [_f32(w) for w in weights]
+    bs = [_f32(b).reshape(-1) for b in biases]
+    f = _f32(feature).reshape(-1)
+    He, L, Fr = Ws[0].shape[0], Ws[3].shape[0], f.shape[0]
+    for w, b, s in zip(Ws, bs, [(He, Fr + 2), (He, He), (He, He), (L, He)]):
+        assert w.shape == s and b.shape == (s[0],), (w.shape, b.shape, s)
+    dims = _EncDims(Fr, He, L)
+    Wp = (C.c_void_p * 4)(*[w.ctypes.data for w in Ws])
+    bp = (C.c_void_p * 4)(*[b.ctypes.data for b in bs])
+    out = np.empty(L, dtype=np.float64)
+    rc = _load().oracle_encode_latent(C.byref(dims), Wp, bp, f.ctypes.data, float(alpha), float(beta), out.ctypes.data)
+    assert rc == 0
     return out

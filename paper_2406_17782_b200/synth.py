@@ -263,3 +263,26 @@ def pd_config(kind, n=None, width=None, height=None, H=64, seed=None, M=8):
         back["rgb"] = (0.3, 0.35, 0.4)
         out["lights"] = np.concatenate([lights_direct5(), back])
     return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# Inputs for the encoder tail.  Data only, as above.
+def enc_layer_shapes(feat_width=256, hidden=128, latent=PD_LATENT):
+    """in-projection, the two fully connected layers of the residual block, out-projection"""
+    return [(hidden, feat_width + 2), (hidden, hidden), (hidden, hidden), (latent, hidden)]
+
+
+def enc_config(feat_width=256, hidden=128, latent=PD_LATENT, seed=21, n_materials=8):
+    """Xavier-uniform fp32 weights, biases 0.01*N(0,1); per material a stand-in for the ResNet-18 feature of its pattern
+    textures (|N(0,1)|: post-ReLU, pooled features are non-negative) and appearance parameters roughness alpha ~ U(0.1, 0.9),
+    height-field scaling beta ~ U(0.5, 2).  Draw order: E0,b0,...,E3,b3; features; alpha; beta."""
+    rng = np.random.default_rng(seed)
+    Ws, bs = [], []
+    for (n_out, n_in) in enc_layer_shapes(feat_width, hidden, latent):
+        a = math.sqrt(6.0 / (n_in + n_out))
+        Ws.append(rng.uniform(-a, a, size=(n_out, n_in)).astype(np.float32))
+        bs.append((0.01 * rng.standard_normal(n_out)).astype(np.float32))
+    feats = np.abs(rng.standard_normal((n_materials, feat_width))).astype(np.float32)
+    alpha = rng.uniform(0.1, 0.9, n_materials).astype(np.float32)
+    beta = rng.uniform(0.5, 2.0, n_materials).astype(np.float32)
+    return {"weights": Ws, "biases": bs, "features": feats, "alpha": alpha, "beta": beta}

@@ -128,6 +128,31 @@ int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, const float*
  * Rows outside [0, max_materials) => NBSDF_E_INVALID. */
 int nbsdf_lerp_latents(nbsdf_ctx* ctx, int32_t dst, int32_t a, int32_t b, float t, void* cuda_stream);
 
+/* ---- Encoder tail on the device (sec. 4.2 "Encoder", 168 Fig. 3 caption; editing path PAPER.md:198) ----
+ * The fully connected residual block that turns a pre-computed ResNet feature of the fabric pattern plus the appearance
+ * parameters (roughness alpha, height-field scaling beta) into a material latent vector (DESIGN.md sec. 12 for the
+ * readings): x = [feature(Fr), alpha, beta];
+ *   e0 = lrelu(W[0] x + b[0]);  r = lrelu(W[1] e0 + b[1]);  e2 = lrelu(W[2] r + b[2] + e0);  z = W[3] e2 + b[3]
+ * with leaky-ReLU slope 0.01, all in fp32.  HOST pointers, fp32, row-major [out][in]:
+ * W[0]: He x (Fr+2), W[1], W[2]: He x He, W[3]: L x He with L = the context's latent_dim.
+ * Supported: hidden He in {32, 64, 128, 256}, 0 <= feat_width Fr <= 1022; else NBSDF_E_UNSUPPORTED. */
+typedef struct {
+    const float* W[4];
+    const float* b[4];
+    int32_t feat_width; /* Fr */
+    int32_t hidden;     /* He: 128 in the paper */
+} nbsdf_encoder_weights;
+
+/* Installs (or replaces) the encoder tail of a context: weights are copied to the device before the call returns
+ * (a set-up call: it synchronises with the device).  Works on contexts made by nbsdf_create or nbsdf_create_paper. */
+int nbsdf_set_encoder(nbsdf_ctx* ctx, const nbsdf_encoder_weights* weights);
+
+/* Runs the encoder tail for one material and writes the result into row `row` of the latent table: one small kernel
+ * enqueued on cuda_stream, ordered like nbsdf_set_latents (visible to every later launch on the stream; no host round
+ * trip, no synchronisation).  feature_host: HOST, Fr fp32, copied before return.  NBSDF_E_INVALID if no encoder has
+ * been installed or row is out of range. */
+int nbsdf_encode_latent(nbsdf_ctx* ctx, int32_t row, const float* feature_host, float alpha, float beta, void* cuda_stream);
+
 /* Batched decoder inference: stages A1-A4, B1-B7 of DESIGN.md in one fused kernel.
  * q_dev: DEVICE, n records, 16-byte aligned.  frames_dev: DEVICE [n][6] = (normal, tangent hint) per query in
  * the space of wi/wo, or NULL when wi/wo are already local.  rgb_dev: DEVICE [n][3] fp32, 16-byte aligned.

@@ -15,7 +15,8 @@ NBSDF_PREC_FP32, NBSDF_PREC_BF16, NBSDF_PREC_FP16 = 0, 1, 2
 PRECISIONS = {"fp32": NBSDF_PREC_FP32, "bf16": NBSDF_PREC_BF16, "fp16": NBSDF_PREC_FP16}
 NBSDF_MAX_LIGHTS = 32
 EXPORTS = ["nbsdf_create", "nbsdf_set_latents", "nbsdf_eval", "nbsdf_shade_frame", "nbsdf_destroy",
-           "nbsdf_last_error", "nbsdf_launch_count", "nbsdf_create_paper", "nbsdf_set_albedos", "nbsdf_lerp_latents"]
+           "nbsdf_last_error", "nbsdf_launch_count", "nbsdf_create_paper", "nbsdf_set_albedos", "nbsdf_lerp_latents",
+           "nbsdf_set_encoder", "nbsdf_encode_latent"]
 
 
 class NbsdfError(RuntimeError):
@@ -35,6 +36,10 @@ class _Weights(C.Structure):
 
 class _PaperWeights(C.Structure):
     _fields_ = [("W", C.c_void_p * 7), ("b", C.c_void_p * 7)]
+
+
+class _EncoderWeights(C.Structure):
+    _fields_ = [("W", C.c_void_p * 4), ("b", C.c_void_p * 4), ("feat_width", C.c_int32), ("hidden", C.c_int32)]
 
 
 class _GBuffer(C.Structure):
@@ -71,6 +76,10 @@ def load():
         lib.nbsdf_lerp_latents.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_void_p]
         lib.nbsdf_set_albedos.restype = C.c_int
         lib.nbsdf_set_albedos.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+        lib.nbsdf_set_encoder.restype = C.c_int
+        lib.nbsdf_set_encoder.argtypes = [C.c_void_p, C.POINTER(_EncoderWeights)]
+        lib.nbsdf_encode_latent.restype = C.c_int
+        lib.nbsdf_encode_latent.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
         _lib = lib
     return _lib
 
@@ -135,6 +144,26 @@ def nbsdf_set_latents(ctx, first, latents_host, stream=None):
     z = np.ascontiguousarray(latents_host, dtype=np.float32)
     z = z.reshape(1, -1) if z.ndim == 1 else z
     _check(load().nbsdf_set_latents(ctx, first, z.shape[0], z.ctypes.data, _stream(stream)), ctx)
+
+
+def nbsdf_set_encoder(ctx, weights, biases):
+    """Encoder tail (include/nbsdf.h): 4 host arrays each, E0 [He][Fr+2], E1, E2 [He][He], E3 [L][He], fp32."""
+    Ws = [np.ascontiguousarray(w, dtype=np.float32) for w in weights]
+    bs = [np.ascontiguousarray(b, dtype=np.float32).reshape(-1) for b in biases]
+    if len(Ws) != 4 or len(bs) != 4:
+        raise ValueError("encoder tail: 4 layers")
+    He, Fr, L = Ws[0].shape[0], Ws[0].shape[1] - 2, Ws[3].shape[0]
+    for w, b, s in zip(Ws, bs, [(He, Fr + 2), (He, He), (He, He), (L, He)]):
+        if w.shape != s or b.shape != (s[0],):
+            raise ValueError(f"layer shape {w.shape}/{b.shape}, expected {s}")
+    ew = _EncoderWeights((C.c_void_p * 4)(*[w.ctypes.data for w in Ws]), (C.c_void_p * 4)(*[b.ctypes.data for b in bs]), Fr, He)
+    _check(load().nbsdf_set_encoder(ctx, C.byref(ew)), ctx)
+
+
+def nbsdf_encode_latent(ctx, row, feature_host, alpha, beta, stream=None):
+    f = np.ascontiguousarray(feature_host, dtype=np.float32).reshape(-1)
+    _check(load().nbsdf_encode_latent(ctx, int(row), f.ctypes.data if f.size else None, float(alpha), float(beta),
+                                      _stream(stream)), ctx)
 
 
 def nbsdf_lerp_latents(ctx, dst, a, b, t, stream=None):

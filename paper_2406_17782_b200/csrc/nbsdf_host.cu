@@ -14,6 +14,9 @@
 namespace nbsdf {
 void pack_fp32(int L, int H, const nbsdf_weights* w, float* blob);
 size_t fp32_blob_floats(int L, int H);
+size_t encoder_blob_floats(int Fr, int He, int L);
+void pack_encoder(int Fr, int He, int L, const nbsdf_encoder_weights* w, float* blob);
+cudaError_t launch_encode_latent(const float* w, const float* x_in, int Fr, int He, int L, float* z_row, cudaStream_t s);
 }  // namespace nbsdf
 
 using namespace nbsdf;
@@ -35,6 +38,10 @@ struct nbsdf_ctx {
     int ring_next = 0;
     int arch = 0;                     // 0: BASELINE.json decoder (nbsdf_create), 1: paper-structured (nbsdf_create_paper)
     float* d_albedos = nullptr;       // arch 1: [M][12] fp32
+    float* d_enc_w = nullptr;         // encoder tail (nbsdf_set_encoder): transposed weights + biases
+    float* d_enc_in = nullptr;        // kRingSlots x kEncInFloats: [feature, alpha, beta] of the in-flight encode calls
+    int enc_fr = -1, enc_he = 0;
+    static constexpr int kEncInFloats = 1024;
     int64_t launches = 0;
     std::string err;
 };
@@ -74,7 +81,9 @@ static cudaError_t ring_create(nbsdf_ctx* ctx, size_t slot_floats)
 }
 
 // host rows -> next pinned slot -> cudaMemcpyAsync to dst on stream s; never waits unless the ring has wrapped
-static cudaError_t ring_upload(nbsdf_ctx* ctx, float* dst, const float* src_host, size_t n_floats, cudaStream_t s)
+static cudaError_t ring_upload(nbsdf_ctx* ctx, float* dst, const float* src_host, size_t n_floats, cudaStream_t s,
+                               const float* tail = nullptr, size_t n_tail = 0, float* dst_slots = nullptr, size_t dst_stride = 0,
+                               int* slot_out = nullptr)
 {
     const int i = ctx->ring_next;
     ctx->ring_next = (i + 1) % nbsdf_ctx::kRingSlots;
@@ -84,8 +93,11 @@ static cudaError_t ring_upload(nbsdf_ctx* ctx, float* dst, const float* src_host
         ctx->ring_busy[i] = false;
     }
     float* slot = ctx->h_ring + (size_t)i * ctx->ring_slot_floats;
-    memcpy(slot, src_host, n_floats * sizeof(float));
-    cudaError_t e = cudaMemcpyAsync(dst, slot, n_floats * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (n_floats) memcpy(slot, src_host, n_floats * sizeof(float));
+    if (n_tail) memcpy(slot + n_floats, tail, n_tail * sizeof(float));
+    if (dst_slots) dst = dst_slots + (size_t)i * dst_stride;      // one device slot per ring slot
+    if (slot_out) *slot_out = i;
+    cudaError_t e = cudaMemcpyAsync(dst, slot, (n_floats + n_tail) * sizeof(float), cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return e;
     e = cudaEventRecord(ctx->ring_ev[i], s);
     if (e == cudaSuccess) ctx->ring_busy[i] = true;
@@ -206,7 +218,7 @@ extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weight
 
     NBSDF_TRY(cudaMalloc(&ctx->d_latents, (size_t)M * L * sizeof(float)), "cudaMalloc(latents)");
     NBSDF_TRY(cudaMemset(ctx->d_latents, 0, (size_t)M * L * sizeof(float)), "cudaMemset(latents)");
-    NBSDF_TRY(ring_create(ctx, (size_t)M * L), "pinned staging ring");
+    NBSDF_TRY(ring_create(ctx, (size_t)M * L > nbsdf_ctx::kEncInFloats ? (size_t)M * L : nbsdf_ctx::kEncInFloats), "pinned staging ring");
     if (cfg->precision == NBSDF_PREC_FP32) {
         std::vector<float> blob(fp32_blob_floats(L, H));
         pack_fp32(L, H, weights, blob.data());
@@ -303,7 +315,7 @@ extern "C" int nbsdf_create_paper(const nbsdf_config* cfg, const nbsdf_paper_wei
     } while (0)
     NBSDF_TRY(cudaMalloc(&ctx->d_latents, (size_t)M * L * sizeof(float)), "cudaMalloc(latents)");
     NBSDF_TRY(cudaMemset(ctx->d_latents, 0, (size_t)M * L * sizeof(float)), "cudaMemset(latents)");
-    NBSDF_TRY(ring_create(ctx, (size_t)M * L), "pinned staging ring");      // L = 64 > 12: one slot also fits M albedo rows
+    NBSDF_TRY(ring_create(ctx, (size_t)M * L > nbsdf_ctx::kEncInFloats ? (size_t)M * L : nbsdf_ctx::kEncInFloats), "pinned staging ring");
     NBSDF_TRY(cudaMalloc(&ctx->d_albedos, (size_t)M * 12 * sizeof(float)), "cudaMalloc(albedos)");
     NBSDF_TRY(cudaMemset(ctx->d_albedos, 0, (size_t)M * 12 * sizeof(float)), "cudaMemset(albedos)");
     {
@@ -344,6 +356,8 @@ extern "C" void nbsdf_destroy(nbsdf_ctx* ctx)
         if (ctx->ring_ev[i]) cudaEventDestroy(ctx->ring_ev[i]);
     }
     if (ctx->h_ring) cudaFreeHost(ctx->h_ring);
+    if (ctx->d_enc_w) cudaFree(ctx->d_enc_w);
+    if (ctx->d_enc_in) cudaFree(ctx->d_enc_in);
     if (ctx->d_albedos) cudaFree(ctx->d_albedos);
     if (ctx->arch == 1) ctx->d_wimg_shade = nullptr;      // alias of d_wimg_eval
     if (ctx->d_latents) cudaFree(ctx->d_latents);
@@ -372,6 +386,56 @@ extern "C" int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, c
     if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
     const cudaError_t e = ring_upload(ctx, ctx->d_latents + (size_t)first * L, latents_host, (size_t)count * L, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_set_latents upload", e);
+    return NBSDF_OK;
+}
+
+extern "C" int nbsdf_set_encoder(nbsdf_ctx* ctx, const nbsdf_encoder_weights* w)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (!w) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_encoder: NULL weights");
+    for (int l = 0; l < 4; ++l)
+        if (!w->W[l] || !w->b[l]) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_encoder: NULL weight or bias pointer");
+    const int Fr = w->feat_width, He = w->hidden, L = ctx->cfg.latent_dim;
+    if (!(He == 32 || He == 64 || He == 128 || He == 256) || Fr < 0 || Fr + 2 > nbsdf_ctx::kEncInFloats)
+        return fail(ctx, NBSDF_E_UNSUPPORTED, "nbsdf_set_encoder: supported are hidden in {32,64,128,256}, 0 <= feat_width <= 1022");
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    std::vector<float> blob(encoder_blob_floats(Fr, He, L));
+    pack_encoder(Fr, He, L, w, blob.data());
+    cudaError_t e = cudaDeviceSynchronize();                // an earlier encode call may still read the old weights
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaDeviceSynchronize", e);
+    if (ctx->d_enc_w) cudaFree(ctx->d_enc_w);
+    ctx->d_enc_w = nullptr;
+    ctx->enc_fr = -1;
+    e = cudaMalloc(&ctx->d_enc_w, blob.size() * sizeof(float));
+    if (e == cudaSuccess && !ctx->d_enc_in)
+        e = cudaMalloc(&ctx->d_enc_in, (size_t)nbsdf_ctx::kRingSlots * nbsdf_ctx::kEncInFloats * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_enc_w, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(ctx, NBSDF_E_NOMEM, "nbsdf_set_encoder: out of device memory")
+                                                                 : fail_cuda(ctx, "nbsdf_set_encoder upload", e);
+    ctx->enc_fr = Fr;
+    ctx->enc_he = He;
+    return NBSDF_OK;
+}
+
+extern "C" int nbsdf_encode_latent(nbsdf_ctx* ctx, int32_t row, const float* feature_host, float alpha, float beta, void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (ctx->enc_fr < 0) return fail(ctx, NBSDF_E_INVALID, "nbsdf_encode_latent: no encoder installed (nbsdf_set_encoder)");
+    if (row < 0 || row >= ctx->cfg.max_materials) return fail(ctx, NBSDF_E_INVALID, "nbsdf_encode_latent: row out of range");
+    if (ctx->enc_fr > 0 && !feature_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_encode_latent: NULL feature");
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const float ab[2] = { alpha, beta };
+    int slot = 0;
+    cudaError_t e = ring_upload(ctx, nullptr, feature_host, (size_t)ctx->enc_fr, s, ab, 2, ctx->d_enc_in, nbsdf_ctx::kEncInFloats, &slot);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_encode_latent upload", e);
+    const int L = ctx->cfg.latent_dim;
+    e = launch_encode_latent(ctx->d_enc_w, ctx->d_enc_in + (size_t)slot * nbsdf_ctx::kEncInFloats, ctx->enc_fr, ctx->enc_he, L,
+                             ctx->d_latents + (size_t)row * L, s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_encode_latent launch", e);
+    ctx->launches += 1;
     return NBSDF_OK;
 }
 

@@ -1,0 +1,100 @@
+"""Encoder tail on the device (nbsdf_set_encoder / nbsdf_encode_latent) against its oracle,
+THROUGH rendering: latents are produced on the device by the encoder kernel, the decoder / frame kernel then runs on
+them, and the result is compared with the oracle decoder evaluated on the ORACLE's encoded latents.  -m gpu."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_2406_17782_b200 import api, synth  # noqa: E402
+
+from test_gpu_parity import Ctx, check  # noqa: E402
+
+
+def oracle_latents(enc, alpha=None, beta=None):
+    alpha = enc["alpha"] if alpha is None else alpha
+    beta = enc["beta"] if beta is None else beta
+    return np.stack([oracle.encode_latent(enc["weights"], enc["biases"], enc["features"][m], alpha[m], beta[m])
+                     for m in range(len(alpha))]).astype(np.float32)
+
+
+@pytest.mark.parametrize("prec", ["fp32", "fp16"])
+@pytest.mark.parametrize("L,He,Fr", [(16, 128, 256), (32, 64, 100), (8, 256, 0)])
+def test_encode_then_eval_matches_oracle(prec, L, He, Fr):
+    cfg = synth.config(1, n=3000, L=L, H=64, seed=40 + L)
+    enc = synth.enc_config(feat_width=Fr, hidden=He, latent=L, seed=21 + L)
+    c = Ctx(cfg, prec, L=L)                                   # latent table starts with cfg's latents ...
+    api.nbsdf_set_encoder(c.ctx, enc["weights"], enc["biases"])
+    for m in range(8):                                        # ... and every row is then replaced by the encoder
+        api.nbsdf_encode_latent(c.ctx, m, enc["features"][m], enc["alpha"][m], enc["beta"][m])
+    out = c.eval(cfg["queries"])
+    c.close()
+    Z = oracle_latents(enc)
+    assert np.abs(Z).max() > 0.1
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], Z, cfg["queries"])
+    check(out, ref, prec, f"encode -> eval L={L} He={He} Fr={Fr}")
+
+
+def test_edit_alpha_beta_reencode_and_shade_paper_context():
+    """The editing path of PAPER.md:198 on the paper-structured decoder: frame 1, edit (alpha, beta) of material 3,
+    re-encode ON THE DEVICE, frame 2; both frames against the oracle, untouched materials bit-identical."""
+    cfg = synth.pd_config("frame", width=320, height=136)
+    enc = synth.enc_config(feat_width=256, hidden=128, latent=64, seed=33)
+    ctx = api.nbsdf_create_paper(cfg["weights"], cfg["biases"], 64, 8, "fp16")
+    api.nbsdf_set_albedos(ctx, 0, cfg["albedos"])
+    api.nbsdf_set_encoder(ctx, enc["weights"], enc["biases"])
+    for m in range(8):
+        api.nbsdf_encode_latent(ctx, m, enc["features"][m], enc["alpha"][m], enc["beta"][m])
+    g, lights = cfg["gbuffer"], cfg["lights"]
+    gd = api.gbuffer_to_device(g)
+    npx = g["width"] * g["height"]
+    f1 = torch.empty((npx, 3), dtype=torch.float32, device="cuda")
+    f2 = torch.empty((npx, 3), dtype=torch.float32, device="cuda")
+    api.nbsdf_shade_frame(ctx, gd, lights, f1)
+    alpha, beta = enc["alpha"].copy(), enc["beta"].copy()
+    alpha[3], beta[3] = 0.15, 1.9
+    api.nbsdf_encode_latent(ctx, 3, enc["features"][3], alpha[3], beta[3])       # no synchronisation in between
+    api.nbsdf_shade_frame(ctx, gd, lights, f2)
+    torch.cuda.synchronize()
+    api.nbsdf_destroy(ctx)
+    f1, f2 = f1.cpu().numpy(), f2.cpu().numpy()
+    ref1 = oracle.pd_shade_frame(cfg["weights"], cfg["biases"], oracle_latents(enc), cfg["albedos"], g, lights)
+    ref2 = oracle.pd_shade_frame(cfg["weights"], cfg["biases"], oracle_latents(enc, alpha, beta), cfg["albedos"], g, lights)
+    check(f1, ref1, "fp16", "frame 1 (encoded latents)")
+    check(f2, ref2, "fp16", "frame 2 (material 3 re-encoded)")
+    same = g["material"] != 3
+    np.testing.assert_array_equal(f1[same].view(np.uint32), f2[same].view(np.uint32))
+    assert (f1[~same] != f2[~same]).any()
+
+
+def test_encoder_errors_and_latency():
+    cfg = synth.config(1, n=64)
+    enc = synth.enc_config(feat_width=256, hidden=128, latent=16)
+    c = Ctx(cfg, "fp16")
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_encode_latent(c.ctx, 0, enc["features"][0], 0.5, 1.0)          # no encoder installed
+    assert e.value.status == api.NBSDF_E_INVALID
+    bad = synth.enc_config(feat_width=16, hidden=48, latent=16)
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_set_encoder(c.ctx, bad["weights"], bad["biases"])
+    assert e.value.status == api.NBSDF_E_UNSUPPORTED
+    api.nbsdf_set_encoder(c.ctx, enc["weights"], enc["biases"])
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_encode_latent(c.ctx, 8, enc["features"][0], 0.5, 1.0)
+    assert e.value.status == api.NBSDF_E_INVALID
+    for i in range(20):
+        api.nbsdf_encode_latent(c.ctx, i % 8, enc["features"][i % 8], 0.5, 1.0)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(200):
+        api.nbsdf_encode_latent(c.ctx, i % 8, enc["features"][i % 8], 0.5, 1.0)
+    e1.record()
+    torch.cuda.synchronize()
+    us = 1e3 * e0.elapsed_time(e1) / 200
+    print(f"encoder tail (Fr=256, He=128, L=16): {us:.1f} us per nbsdf_encode_latent (paper: ~0.5 ms incl. the ResNet trunk)")
+    assert us < 500.0
+    c.close()

@@ -74,6 +74,9 @@ def _load():
         lib.oracle_pd_shade_frame.restype = C.c_int
         lib.oracle_pd_shade_frame.argtypes = [C.c_void_p] * 9 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
                                                                  C.c_int, C.c_void_p, C.c_int]
+        lib.oracle_pd_shade_frame_px.restype = C.c_int
+        lib.oracle_pd_shade_frame_px.argtypes = [C.c_void_p] * 10 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                                                     C.c_int, C.c_void_p, C.c_int]
         lib.oracle_encode_latent.restype = C.c_int
         lib.oracle_encode_latent.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p]
         global _all_threads
@@ -215,7 +218,8 @@ def pd_eval_queries(weights, biases, latents, albedos, queries, frames=None, n_t
 
 
 def pd_shade_frame(weights, biases, latents, albedos, gbuffer, lights, first=0, count=None, n_threads=0):
-    """fp64 frame shading with the paper-structured decoder (|cos| weighting; pos_fp.w = footprint size)."""
+    """fp64 frame shading with the paper-structured decoder (|cos| weighting; pos_fp.w = footprint size).
+    gbuffer may carry "albedo": a per-pixel plane [h*w][12] that replaces the material's table row."""
     dims, Wp, bp, Z, A, _keep = _pack_pd(weights, biases, latents, albedos)
     pos = _f32(gbuffer["pos_fp"]).reshape(-1, 4)
     nrm = _f32(gbuffer["nrm_u"]).reshape(-1, 4)
@@ -229,10 +233,15 @@ def pd_shade_frame(weights, biases, latents, albedos, gbuffer, lights, first=0, 
     assert 0 <= first and first + count <= npx
     assert npx == 0 or int(mat.max()) < Z.shape[0], "material id out of range"
     out = np.empty((count, 3), dtype=np.float64)
-    rc = _load().oracle_pd_shade_frame(C.byref(dims), Wp, bp, Z.ctypes.data, A.ctypes.data, pos.ctypes.data,
-                                       nrm.ctypes.data, tan.ctypes.data, mat.ctypes.data, first, count,
-                                       cam.ctypes.data, lt.ctypes.data if lt.shape[0] else None, lt.shape[0],
-                                       out.ctypes.data, _threads(n_threads))
+    apx = None
+    if gbuffer.get("albedo") is not None:
+        apx = _f32(gbuffer["albedo"]).reshape(-1, 12)
+        assert apx.shape[0] == npx
+    rc = _load().oracle_pd_shade_frame_px(C.byref(dims), Wp, bp, Z.ctypes.data, A.ctypes.data,
+                                          apx.ctypes.data if apx is not None else None, pos.ctypes.data,
+                                          nrm.ctypes.data, tan.ctypes.data, mat.ctypes.data, first, count,
+                                          cam.ctypes.data, lt.ctypes.data if lt.shape[0] else None, lt.shape[0],
+                                          out.ctypes.data, _threads(n_threads))
     assert rc == 0
     return out
 

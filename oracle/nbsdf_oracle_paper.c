@@ -208,11 +208,14 @@ int oracle_pd_eval(const oracle_pd_dims* d, const float* const W[7], const float
     return 0;
 }
 
-/* Frame shading with the paper-structured decoder: as oracle_shade_frame, but L += f * E * |wi_local.z|. */
-int oracle_pd_shade_frame(const oracle_pd_dims* d, const float* const W[7], const float* const b[7], const float* Z,
-                          const float* albedos, const float* pos_fp, const float* nrm_u, const float* tan_v,
-                          const int32_t* material, int64_t first, int64_t count, const float cam_pos[3],
-                          const oracle_pd_light* lights, int n_lights, double* out, int n_threads)
+/* Frame shading with the paper-structured decoder: as oracle_shade_frame, but L += f * E * |wi_local.z|.
+ * albedo_px: NULL, or a per-pixel albedo plane [h*w][12] (kd_warp, kd_weft, ks_warp, ks_weft, RGB each) that replaces the
+ * material's table row in Eq. 8 for that pixel -- "spatial-varying appearances when applying albedo maps, by computing
+ * k_d and k_s via mipmapping": the mip-mapped fetch is the renderer's, its result is this plane. */
+int oracle_pd_shade_frame_px(const oracle_pd_dims* d, const float* const W[7], const float* const b[7], const float* Z,
+                             const float* albedos, const float* albedo_px, const float* pos_fp, const float* nrm_u,
+                             const float* tan_v, const int32_t* material, int64_t first, int64_t count,
+                             const float cam_pos[3], const oracle_pd_light* lights, int n_lights, double* out, int n_threads)
 {
     if (!d || !W || !b || !Z || !albedos || count < 0 || n_lights < 0) return -1;
     if (count > 0 && (!pos_fp || !nrm_u || !tan_v || !material || !out || !cam_pos)) return -1;
@@ -267,7 +270,7 @@ int oracle_pd_shade_frame(const oracle_pd_dims* d, const float* const W[7], cons
                 double wi_loc[3], comp[4], rgb[3];
                 oracle_to_local(nn, tt, wi, wi_loc);
                 pd_components(d, W, b, Z, m, u, v, size, wi_loc, wo_loc, scratch, comp);
-                pd_combine(albedos + 12 * (size_t)m, comp, rgb);
+                pd_combine(albedo_px ? albedo_px + 12 * (size_t)p : albedos + 12 * (size_t)m, comp, rgb);
                 const double c = fabs(wi_loc[2]);
                 for (int i = 0; i < 3; ++i) Lp[i] += rgb[i] * E[i] * c;
             }
@@ -275,6 +278,15 @@ int oracle_pd_shade_frame(const oracle_pd_dims* d, const float* const W[7], cons
         free(scratch);
     }
     return 0;
+}
+
+int oracle_pd_shade_frame(const oracle_pd_dims* d, const float* const W[7], const float* const b[7], const float* Z,
+                          const float* albedos, const float* pos_fp, const float* nrm_u, const float* tan_v,
+                          const int32_t* material, int64_t first, int64_t count, const float cam_pos[3],
+                          const oracle_pd_light* lights, int n_lights, double* out, int n_threads)
+{
+    return oracle_pd_shade_frame_px(d, W, b, Z, albedos, NULL, pos_fp, nrm_u, tan_v, material, first, count, cam_pos, lights,
+                                    n_lights, out, n_threads);
 }
 
 /* Latent interpolation / extrapolation (sec. 6.3): z = (1 - t) z_a + t z_b, t any real ("the material

@@ -298,6 +298,32 @@ def test_frame_shading_emitter_cosine_closed_form():
     np.testing.assert_allclose(oracle.pd_shade_frame(*args, g, lt, first=0, count=1), iso * np.float64(np.float32(0.8)), rtol=1e-13)
 
 
+def test_per_pixel_albedo_plane():
+    """PAPER.md:261 / Eq. 8 per pixel: a plane that repeats each pixel's material row reproduces the table path bit for
+    bit; a basis plane extracts one component per pixel; the frame is linear in the plane; the table is ignored when a
+    plane is given."""
+    cfg = synth.pd_config("frame", width=8, height=4, seed=13)
+    args = (cfg["weights"], cfg["biases"], cfg["latents"])
+    g, lt = dict(cfg["gbuffer"]), cfg["lights"]
+    base = oracle.pd_shade_frame(*args, cfg["albedos"], g, lt)
+    g["albedo"] = cfg["albedos"][g["material"]]
+    np.testing.assert_array_equal(oracle.pd_shade_frame(*args, cfg["albedos"], g, lt), base)
+    np.testing.assert_array_equal(oracle.pd_shade_frame(*args, np.zeros_like(cfg["albedos"]), g, lt), base)   # table unused
+    rng = np.random.default_rng(2)
+    A1 = rng.uniform(0.1, 0.9, (32, 12)).astype(np.float32)
+    A2 = rng.uniform(0.1, 0.9, (32, 12)).astype(np.float32)
+    f = lambda A: oracle.pd_shade_frame(*args, cfg["albedos"], dict(g, albedo=A), lt)          # noqa: E731
+    np.testing.assert_allclose(f(A1.astype(np.float64) + A2), f(A1) + f(A2), rtol=2e-7)          # fp32 storage of the sum
+    # pixel 5 gets kd_warp = (1, 0, 0) and nothing else: its red channel is sum_l C_warp E_r |cos|, green and blue vanish
+    B = np.zeros((32, 12), np.float32)
+    B[5, 0] = 1.0
+    out = f(B)
+    assert out[5, 0] > 0 and out[5, 1] == 0 and out[5, 2] == 0 and (np.delete(out, 5, 0) == 0).all()
+    g["material"] = g["material"].copy()
+    g["material"][5] = -1
+    assert (oracle.pd_shade_frame(*args, cfg["albedos"], dict(g, albedo=B), lt)[5] == 0).all()   # background stays black
+
+
 def test_lerp_latent_closed_forms():
     """interpolation and extrapolation of two material latent vectors."""
     za = np.array([1.0, -2.0, 0.5, 8.0], np.float32)

@@ -90,7 +90,7 @@ typedef struct {
     float wo[3];      /* to the viewer */
 } nbsdf_query;
 
-/* Headless G-buffer, DEVICE planes, 52 bytes per pixel; pixel index = y * width + x. */
+/* Headless G-buffer, DEVICE planes, 52 bytes per pixel (+ 48 with an albedo plane); pixel index = y * width + x. */
 typedef struct {
     const float* pos_fp;     /* [h*w][4]: world x, y, z, footprint   (16-byte aligned) */
     const float* nrm_u;      /* [h*w][4]: shading normal nx, ny, nz, u               */
@@ -98,6 +98,11 @@ typedef struct {
     const int32_t* material; /* [h*w]; < 0 = background => radiance (0,0,0)          */
     int32_t width, height;
     float cam_pos[3];        /* pinhole position; wo = normalize(cam_pos - x)        */
+    const float* albedo;     /* NULL, or (contexts made by nbsdf_create_paper only) [h*w][12]: per-pixel kd_warp, kd_weft,
+                              * ks_warp, ks_weft (RGB each) that replace the material's row of the albedo table in Eq. 8 --
+                              * "spatial-varying appearances when applying albedo maps, by computing k_d and k_s via
+                              * mipmapping"; the mip-mapped texture fetch is the renderer's, its result is
+                              * this plane.  16-byte aligned.  Non-NULL on an nbsdf_create context => NBSDF_E_INVALID. */
 } nbsdf_gbuffer;
 
 /* type 0: directional, vec = direction TO the light (normalised by the library), rgb = radiance E.

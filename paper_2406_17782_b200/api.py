@@ -44,7 +44,7 @@ class _EncoderWeights(C.Structure):
 
 class _GBuffer(C.Structure):
     _fields_ = [("pos_fp", C.c_void_p), ("nrm_u", C.c_void_p), ("tan_v", C.c_void_p), ("material", C.c_void_p),
-                ("width", C.c_int32), ("height", C.c_int32), ("cam_pos", C.c_float * 3)]
+                ("width", C.c_int32), ("height", C.c_int32), ("cam_pos", C.c_float * 3), ("albedo", C.c_void_p)]
 
 
 _lib = None
@@ -179,7 +179,8 @@ def nbsdf_shade_frame(ctx, gbuf, lights_host, radiance_dev, stream=None):
     """gbuf: dict(pos_fp, nrm_u, tan_v: CUDA float32 [h*w][4]; material: CUDA int32 [h*w]; width; height; cam_pos)."""
     g = _GBuffer(gbuf["pos_fp"].data_ptr(), gbuf["nrm_u"].data_ptr(), gbuf["tan_v"].data_ptr(),
                  gbuf["material"].data_ptr(), int(gbuf["width"]), int(gbuf["height"]),
-                 (C.c_float * 3)(*[float(c) for c in gbuf["cam_pos"]]))
+                 (C.c_float * 3)(*[float(c) for c in gbuf["cam_pos"]]),
+                 gbuf["albedo"].data_ptr() if gbuf.get("albedo") is not None else None)
     lt = np.ascontiguousarray(lights_host, dtype=LIGHT_DTYPE).reshape(-1)
     _check(load().nbsdf_shade_frame(ctx, C.byref(g), lt.ctypes.data if lt.shape[0] else None, lt.shape[0],
                                     _ptr(radiance_dev), _stream(stream)), ctx)
@@ -203,5 +204,7 @@ def queries_to_device(q, device="cuda"):
 def gbuffer_to_device(g, device="cuda"):
     import torch
     out = {k: torch.from_numpy(np.ascontiguousarray(g[k])).to(device) for k in ("pos_fp", "nrm_u", "tan_v", "material")}
+    if g.get("albedo") is not None:
+        out["albedo"] = torch.from_numpy(np.ascontiguousarray(g["albedo"], dtype=np.float32)).to(device)
     out.update(width=g["width"], height=g["height"], cam_pos=[float(c) for c in g["cam_pos"]])
     return out

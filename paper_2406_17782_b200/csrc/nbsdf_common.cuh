@@ -34,6 +34,7 @@ struct FrameParams {
     const float4* nrm_u;
     const float4* tan_v;
     const int32_t* material;
+    const float4* albedo;        // paper-structured contexts: per-pixel [12] albedos (3 float4 per pixel), or NULL
     int64_t n_pixels;
     float cam[3];
 };

@@ -509,8 +509,10 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     if (npx >= ((int64_t)1 << 38)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: width * height must be below 2^38");
     if (!g->pos_fp || !g->nrm_u || !g->tan_v || !g->material || !radiance_dev)
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL buffer");
-    if (!aligned16(g->pos_fp) || !aligned16(g->nrm_u) || !aligned16(g->tan_v) || !aligned16(radiance_dev))
+    if (!aligned16(g->pos_fp) || !aligned16(g->nrm_u) || !aligned16(g->tan_v) || !aligned16(radiance_dev) || !aligned16(g->albedo))
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: planes and output must be 16-byte aligned");
+    if (g->albedo && ctx->arch != 1)
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: an albedo plane needs a context made by nbsdf_create_paper");
     for (int l = 0; l < n_lights; ++l)
         if (lights_host[l].type != 0 && lights_host[l].type != 1)
             return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: light type must be 0 (directional) or 1 (point)");
@@ -535,6 +537,7 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     fr.nrm_u = reinterpret_cast<const float4*>(g->nrm_u);
     fr.tan_v = reinterpret_cast<const float4*>(g->tan_v);
     fr.material = g->material;
+    fr.albedo = reinterpret_cast<const float4*>(g->albedo);
     fr.n_pixels = npx;
     fr.cam[0] = g->cam_pos[0]; fr.cam[1] = g->cam_pos[1]; fr.cam[2] = g->cam_pos[2];
     const NetParams net = net_params(ctx);

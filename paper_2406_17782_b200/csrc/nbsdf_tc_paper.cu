@@ -283,32 +283,59 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         for (int c = 0; c < 3; ++c) w_nxt[c] = E[c] * cs;
     };
 
-    // output stage: four raw outputs -> components (inverse log map) -> Eq. 8 with the material's albedos
-    float o_prev[4] = { 0.0f, 0.0f, 0.0f, 0.0f }, rad[3] = { 0.0f, 0.0f, 0.0f };
-    auto bsdf_rgb = [&](int m, float kinv, float rgb[3]) {
-        const float4* al = reinterpret_cast<const float4*>(g_alb + 12 * (m < 0 ? 0 : m));
-        const float4 a0 = al[0], a1 = al[1], a2 = al[2];            // kd_warp rgb, kd_weft rgb, ks_warp rgb, ks_weft rgb
-        const float cw = o_prev[0], cf = o_prev[1];
-        const float sw = fast_expm1(o_prev[2]) * kinv, sf = fast_expm1(o_prev[3]) * kinv;
-        rgb[0] = a0.x * cw + a0.w * cf + a1.z * sw + a2.y * sf;
-        rgb[1] = a0.y * cw + a1.x * cf + a1.w * sw + a2.z * sf;
-        rgb[2] = a0.z * cw + a1.y * cf + a2.x * sw + a2.w * sf;
+    // output stage: four raw outputs -> components (inverse log map) -> Eq. 8 with the albedos.
+    // Eq. 8 is linear in the components, so the frame kernel accumulates radiance PER COMPONENT over the lights
+    // (radc[j][c] = sum_l comp_j E_c |cos|) and applies the albedos once per pixel at the end -- which is also what lets
+    // the albedos come from a per-pixel plane (k_d, k_s from albedo maps) at one fetch per pixel.
+    float o_prev[4] = { 0.0f, 0.0f, 0.0f, 0.0f };
+    float radc[kShade ? 4 : 1][3];
+#pragma unroll
+    for (int j = 0; j < (kShade ? 4 : 1); ++j) radc[j][0] = radc[j][1] = radc[j][2] = 0.0f;
+    auto components = [&](float kinv, float comp[4]) {
+        comp[0] = o_prev[0];
+        comp[1] = o_prev[1];
+        comp[2] = fast_expm1(o_prev[2]) * kinv;
+        comp[3] = fast_expm1(o_prev[3]) * kinv;
+    };
+    auto accumulate = [&](float kinv) {                   // shade: + components of the light just decoded x E |cos|
+        float comp[4];
+        components(kinv, comp);
+#pragma unroll
+        for (int j = 0; j < (kShade ? 4 : 1); ++j)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) radc[j][c] = fmaf(comp[j], w_cur[c], radc[j][c]);
     };
     int prev_tile = 0;
     int prev_kind = 0, prev_mat = 0;    // kind 0: nothing pending / dead row, 1: store, 2: background (store zeros)
     auto flush_output = [&]() {
         if (prev_kind != 0) {
-            float r[3];
-            bsdf_rgb(prev_mat, kinv_cur, r);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                if (kShade) r[c] = fmaf(r[c], w_cur[c], rad[c]);
-                if (prev_kind == 2) r[c] = 0.0f;
+            float4 a0, a1, a2;                            // kd_warp rgb, kd_weft rgb, ks_warp rgb, ks_weft rgb
+            if (kShade && fr.albedo != nullptr && prev_kind == 1) {
+                const float4* al = fr.albedo + 3 * ((int64_t)prev_tile * 128 + t);
+                a0 = __ldg(al); a1 = __ldg(al + 1); a2 = __ldg(al + 2);
+            } else {
+                const float4* al = reinterpret_cast<const float4*>(g_alb + 12 * (prev_mat < 0 ? 0 : prev_mat));
+                a0 = al[0]; a1 = al[1]; a2 = al[2];
             }
+            float r[3];
+            if constexpr (kShade) {
+                accumulate(kinv_cur);                     // the last light
+                r[0] = a0.x * radc[0][0] + a0.w * radc[1][0] + a1.z * radc[2][0] + a2.y * radc[3][0];
+                r[1] = a0.y * radc[0][1] + a1.x * radc[1][1] + a1.w * radc[2][1] + a2.z * radc[3][1];
+                r[2] = a0.z * radc[0][2] + a1.y * radc[1][2] + a2.x * radc[2][2] + a2.w * radc[3][2];
+            } else {
+                float comp[4];
+                components(kinv_cur, comp);
+                r[0] = a0.x * comp[0] + a0.w * comp[1] + a1.z * comp[2] + a2.y * comp[3];
+                r[1] = a0.y * comp[0] + a1.x * comp[1] + a1.w * comp[2] + a2.z * comp[3];
+                r[2] = a0.z * comp[0] + a1.y * comp[1] + a2.x * comp[2] + a2.w * comp[3];
+            }
+            if (prev_kind == 2) r[0] = r[1] = r[2] = 0.0f;
             P.store_rgb(out, prev_tile, r);
         }
         prev_kind = 0;
-        rad[0] = rad[1] = rad[2] = 0.0f;
+#pragma unroll
+        for (int j = 0; j < (kShade ? 4 : 1); ++j) radc[j][0] = radc[j][1] = radc[j][2] = 0.0f;
     };
     auto load_output = [&]() {
         uint32_t o[4];
@@ -361,13 +388,9 @@ pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
             publish();                                    // -> round 3 (also: this thread has read the previous light's output)
             if constexpr (kShade) {                       // shadow: C2 of the previous light
                 if (l > 0) {
-                    float r[3];
-                    bsdf_rgb(mat_cur, kinv_cur, r);
+                    accumulate(kinv_cur);
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        rad[c] = fmaf(r[c], w_cur[c], rad[c]);
-                        w_cur[c] = w_nxt[c];
-                    }
+                    for (int c = 0; c < 3; ++c) w_cur[c] = w_nxt[c];
                     kinv_cur = kinv_nxt;
                 }
             }

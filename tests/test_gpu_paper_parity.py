@@ -157,6 +157,35 @@ def test_paper_frame_with_emitter_normals():
     c.close()
 
 
+def test_paper_frame_per_pixel_albedo_plane():
+    """Eq. 8 per pixel: albedos from a [h*w][12] plane instead of the material table."""
+    cfg = synth.pd_config("frame", width=333, height=97, seed=41)
+    g, lights = cfg["gbuffer"], cfg["lights"]
+    g["material"] = g["material"].copy()
+    g["material"][3::71] = -1
+    rng = np.random.default_rng(5)
+    npx = g["width"] * g["height"]
+    gA = dict(g, albedo=rng.uniform(0.05, 0.95, (npx, 12)).astype(np.float32))
+    ref = oracle.pd_shade_frame(*_args(cfg), gA, lights)
+    c = PCtx(cfg, "fp16")
+    out = c.shade(gA, lights)
+    live = g["material"] >= 0
+    assert (out[~live] == 0).all()
+    check(out[live], ref[live], "paper frame, per-pixel albedos")
+    # a plane that repeats every pixel's table row takes the same arithmetic path: identical bits
+    gT = dict(g, albedo=cfg["albedos"][np.maximum(g["material"], 0)])
+    np.testing.assert_array_equal(c.shade(gT, lights).view(np.uint32), c.shade(g, lights).view(np.uint32))
+    c.close()
+    # the BASELINE.json decoder has no albedos: a plane is rejected there
+    c0 = synth.config(2, width=16, height=8)
+    ctx = api.nbsdf_create(c0["weights"], c0["biases"], 16, 64, 8, "fp16")
+    g0 = dict(c0["gbuffer"], albedo=np.zeros((128, 12), np.float32))
+    with pytest.raises(api.NbsdfError) as e:
+        api.nbsdf_shade_frame(ctx, api.gbuffer_to_device(g0), c0["lights"], torch.empty((128, 3), device="cuda"))
+    assert e.value.status == api.NBSDF_E_INVALID
+    api.nbsdf_destroy(ctx)
+
+
 def test_paper_frame_matches_eval_on_expanded_queries():
     """The frame kernel runs the fusion layers once per pixel; nbsdf_eval on the (pixel, light) list does not."""
     cfg = synth.pd_config("frame", width=64, height=40)

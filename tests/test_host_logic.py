@@ -42,4 +42,4 @@ def test_wire_formats_match_the_header():
     assert [synth.QUERY_DTYPE.fields[k][1] for k in ("u", "v", "footprint", "material", "wi", "wo")] == [0, 4, 8, 12, 16, 28]
     assert [synth.LIGHT_DTYPE.fields[k][1] for k in ("type", "vec", "rgb", "emit_n")] == [0, 4, 16, 28]
     import ctypes as C
-    assert C.sizeof(api._GBuffer) == 4 * 8 + 8 + 12 + 4   # 4 pointers, w, h, cam[3], tail padding to 8
+    assert C.sizeof(api._GBuffer) == 4 * 8 + 8 + 12 + 4 + 8   # 4 pointers, w, h, cam[3], padding to 8, albedo pointer

@@ -21,6 +21,8 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
+#include <type_traits>
+
 #include "nbsdf_probe.cuh"      // NBSDF_STAMP: no-ops unless built with -DNBSDF_PROBE (debug library only)
 #include "nbsdf_tc_pipeline.cuh"
 
@@ -58,6 +60,11 @@ struct Tc {
     // assembly of the next tile stores x and the tail block straight to TMEM and a tile starts without any store
     static constexpr bool kXDirect = kMerged && NWG * (H + kAw + 8 + K1p / 2) <= 504;
     static constexpr int kXCol = H + kAw + 8;
+    // K-split hand-over of the K = H layers (Pipe::publish2), where a 64-column epilogue writes its operand in two
+    // stores.  Measured (profiles/r2_experiments.md sec. 4): +6 % where x shares the A region (L = 32: the tile starts
+    // with a store in its chain), -1.5 % .. -3 % everywhere else (the second barrier costs more than the overlap returns
+    // when the chain is already short), so it is enabled only there.
+    static constexpr bool kSplit = H == 64 && kMerged && !kXDirect && 2 * NWG + 1 <= 15;
     static constexpr int kColsPerWg = kShade ? H + H / 2 + 24 : H + kAw + (kMerged ? 8 : 0) + (kXDirect ? K1p / 2 : 0);
     static constexpr int kOneCol = S::kOneCol;
     static_assert(NWG * kColsPerWg <= kOneCol, "TMEM budget");
@@ -73,8 +80,11 @@ struct Tc {
 // Epilogue of a hidden layer: acc (N fp32 columns, bias already inside) -> (ReLU) -> packed 16-bit pairs -> A columns.
 // kTwoLoads: 64 columns (two tcgen05.ld) are requested per wait, so the second load's latency hides behind the
 // first's; costs 32 more live registers.
-template <int N, bool kRelu, bool kBf16, bool kTwoLoads = true>
-__device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_taddr)
+struct NoMid { __device__ __forceinline__ void operator()() const {} };
+
+// mid(): called between the two stores of a 64-column epilogue (the K-split hand-over, Pipe::publish2)
+template <int N, bool kRelu, bool kBf16, bool kTwoLoads = true, typename Mid = NoMid>
+__device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_taddr, Mid mid = Mid())
 {
     if constexpr (kTwoLoads && N % 64 == 0) {
 #pragma unroll
@@ -88,6 +98,7 @@ __device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_tad
             for (int j = 0; j < 16; ++j)
                 p[j] = pack2<kBf16, kRelu>(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
             tmem_st16(a_taddr + c / 2, p);
+            if (N == 64) mid();
 #pragma unroll
             for (int j = 0; j < 16; ++j)
                 p[j] = pack2<kBf16, kRelu>(__uint_as_float(w[2 * j]), __uint_as_float(w[2 * j + 1]));
@@ -99,6 +110,7 @@ __device__ __forceinline__ void epilogue_to_a(uint32_t acc_taddr, uint32_t a_tad
             uint32_t v[32];
             tmem_ld32(acc_taddr + c, v);
             tmem_wait_ld();
+            if (N == 64 && c == 32) mid();      // the whole accumulator has been read, the first half is stored
             uint32_t p[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j)
@@ -150,6 +162,16 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
     auto row_is_live = [&](int tile) { return P.row_is_live(tile); };
     auto stage_request = [&](int tile, uint32_t k) { P.stage_request(tile, k); };
     auto publish = [&]() { P.publish(); };
+    // epilogue of a 64-wide hidden layer + hand-over of its result as the next layer's operand (K-split where enabled)
+    auto epilogue_publish = [&]() {
+        if constexpr (T::kSplit) {
+            epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t, [&]() { P.publish(); });
+            P.publish2();
+        } else {
+            epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+            P.publish();
+        }
+    };
     auto await_mma = [&]() { P.await_mma(); };
 
     P.wait_prior_grid(fr, net.latents);
@@ -172,6 +194,23 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         // Mirrors the owning warpgroup's static layer sequence: wait for "operand ready", issue the layer, commit.
         // Blocking in tcgen05.mma issue (the tensor pipe's queue is shallow) costs nothing here.
         auto ready = [&]() { P.ready(); };
+        // a K = H layer whose operand arrives in two halves (Pipe::publish2): K steps 0-1 after the first half, the rest
+        // (incl. the bias / tail step at address `last`) and the commit after the second
+        auto issue_hidden = [&](auto n_tag, uint32_t last, uint32_t w) {
+            constexpr int N = decltype(n_tag)::value;
+            ready();
+            if constexpr (T::kSplit) {
+                if (elect_one()) issue_layer<kBf16, H + 16, N, H, 0, 2>(acc_d, ah_d, last, w, mma_bar);
+                __syncwarp();
+                P.ready2();
+                if (elect_one()) issue_layer<kBf16, H + 16, N, H, 2, (H + 16) / 16>(acc_d, ah_d, last, w, mma_bar);
+            } else {
+                if (elect_one()) issue_layer<kBf16, H + 16, N, H>(acc_d, ah_d, last, w, mma_bar);
+            }
+        };
+        using NH = std::integral_constant<int, H>;
+        using N16 = std::integral_constant<int, 16>;
+        using NF = std::integral_constant<int, kFeat>;
         uint32_t k = 0;
         for (int tile = wg < NWG ? first : n_tiles; tile < n_tiles; tile += stride, ++k) {
             ready();
@@ -184,43 +223,30 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                 issue_layer<kBf16, T::K1p, H, T::K1p>(acc_d, T::kXDirect ? col0 + T::kXCol : ay_d, one_d, w_s[0], mma_bar);
             }
             __syncwarp();
-            ready();
-            if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[1], mma_bar);
+            issue_hidden(NH{}, one_d, w_s[1]);
             __syncwarp();
             if constexpr (T::kMerged) {
-                ready();
-                if (elect_one()) issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, col0 + T::kTailCol, w_s[2], mma_bar);
+                issue_hidden(NH{}, col0 + T::kTailCol, w_s[2]);
                 __syncwarp();
                 // the ready() that follows assemble(next) (one round later with kXDirect): staging buffer (k + 1) & 1 is free
-                ready();
-                if (elect_one()) {
-                    issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[3], mma_bar);
-                    if (!T::kXDirect) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
-                }
+                issue_hidden(NH{}, one_d, w_s[3]);
+                if (!T::kXDirect && elect_one()) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
                 __syncwarp();
-                ready();
-                if (elect_one()) {
-                    issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
-                    if (T::kXDirect) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
-                }
+                issue_hidden(N16{}, one_d, w_s[4]);
+                if (T::kXDirect && elect_one()) stage_request(tile + 3 * stride, k + 3u);       // after the MMAs: not in the layer chain
                 __syncwarp();
             } else {
-                ready();
-                if (elect_one()) issue_layer<kBf16, H + 16, kFeat, H>(acc_d, ah_d, one_d, w_s[2], mma_bar);
+                issue_hidden(NF{}, one_d, w_s[2]);
                 __syncwarp();
                 const int n_rounds = kShade ? lights.n : 1;
                 for (int l = 0; l < n_rounds; ++l) {
                     ready();
                     if (elect_one()) issue_layer<kBf16, T::K4p, H, T::K4p>(acc_d, ay_d, one_d, w_s[3], mma_bar);
                     __syncwarp();
-                    ready();                                  // eval: follows assemble(next)
-                    if (elect_one()) {
-                        issue_layer<kBf16, H + 16, H, H>(acc_d, ah_d, one_d, w_s[4], mma_bar);
-                        if (!kShade) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
-                    }
+                    issue_hidden(NH{}, one_d, w_s[4]);        // eval: follows assemble(next)
+                    if (!kShade && elect_one()) stage_request(tile + 3 * stride, k + 3u);      // after the MMAs: not in the layer chain
                     __syncwarp();
-                    ready();
-                    if (elect_one()) issue_layer<kBf16, H + 16, 16, H>(acc_d, ah_d, one_d, w_s[5], mma_bar);
+                    issue_hidden(N16{}, one_d, w_s[5]);
                     __syncwarp();
                 }
             }
@@ -354,29 +380,24 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
         publish();                                        // -> layer 1 (short: nothing is put in its shadow)
         await_mma();
         NBSDF_STAMP(tid == 0 && k == 0, net, 5);
-        epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-        publish();                                        // -> layer 2
+        epilogue_publish();                               // -> layer 2
         flush_output();                                   // shadow of layer 2: the previous tile's B7 / C2-C3
         NBSDF_STAMP(tid == 0 && k == 1, net, 6);
         if constexpr (kShade) light_tail(0);              //                    and C1 of the first light
         await_mma();
-        epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
+        epilogue_publish();                               // -> merged layer / layer 3
 
         if constexpr (T::kMerged) {
             // ---- merged layers 3+4 (B3-B4): (W4f W3) h2 + W4a [wi, wo] + (W4f b3 + b4); K = H from AH + tail block ----
-            publish();                                    // -> merged layer
             if constexpr (!T::kXDirect) assemble(tile + stride, k + 1u);      // shadow of the merged layer: A1-A4 of the next tile
             await_mma();
-            epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-            publish();                                    // -> layer 5
+            epilogue_publish();                           // -> layer 5
             if constexpr (T::kXDirect) assemble(tile + stride, k + 1u);       // shadow of layer 5 (the merged layer is done)
             await_mma();
-            epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-            publish();                                    // -> layer 6
+            epilogue_publish();                           // -> layer 6
             await_mma();
             load_output();
         } else {
-            publish();                                    // -> layer 3
             await_mma();
             epilogue_to_a<kFeat, false, kBf16>(acc_t, ay_t);      // feat (linear) -> AY columns [0, 16)
             store_tail(ay_t + 16);                                // [wi, wo, c] of the query / of light 0
@@ -399,8 +420,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                     assemble(tile + stride, k + 1u);      // shadow of layer 4: A1-A4 of the next tile
                 }
                 await_mma();
-                epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-                publish();                                // -> layer 5; eval: the issuer also refills the staging buffer just read
+                epilogue_publish();                       // -> layer 5; eval: the issuer also refills the staging buffer just read
                 if constexpr (kShade) {                   // shadow of layer 5: C1 of the next light, or A1-A4 of the next tile
                     if (l + 1 < n_rounds) {
                         light_tail(l + 1);
@@ -410,8 +430,7 @@ tc_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restr
                     }
                 }
                 await_mma();
-                epilogue_to_a<H, true, kBf16, T::kTwoLoads>(acc_t, ah_t);
-                publish();                                // -> layer 6
+                epilogue_publish();                       // -> layer 6
                 await_mma();
                 load_output();
             }

@@ -262,6 +262,22 @@ struct Pipe {
         named_bar_sync(1 + wg, 160);
         tc_fence_after();
     }
+    // K-split hand-over (a second named barrier per warpgroup): an epilogue that writes its operand in two halves
+    // publishes the first half with publish() and the second with publish2(); the issuer issues the K steps that read
+    // the first half after ready() and the rest + the commit after ready2(), so the layer's first MMAs run while the
+    // owners still convert the second half.  Legal because every owner has READ the whole accumulator (tcgen05.wait::ld)
+    // before its first arrive, so the first MMA may overwrite it.
+    __device__ __forceinline__ void publish2() const
+    {
+        tmem_wait_st();
+        tc_fence_before();
+        named_bar_arrive(1 + NWG + wg, 160);
+    }
+    __device__ __forceinline__ void ready2() const
+    {
+        named_bar_sync(1 + NWG + wg, 160);
+        tc_fence_after();
+    }
     __device__ __forceinline__ void await_mma()                // owners: the layer committed last has completed
     {
         mbar_wait(mma_bar, mma_phase);

@@ -221,18 +221,20 @@ __host__ __device__ constexpr uint32_t make_idesc(int N)
 // Called by ONE thread.  K/16 steps in total; the first KA/16 read the A operand at a_tmem, the remaining ones
 // (the bias step of the K = H layers) read the constant block at one_tmem.  d_tmem/a_tmem/one_tmem are lane-0
 // TMEM addresses; w_saddr is the layer's weight tiles in shared memory.
-template <bool kBf16, int K, int N, int KA>
+// kS0, kS1: only the K steps [kS0, kS1) are issued (a layer issued in two parts, see Pipe::publish2); the commit goes
+// with the part that ends at K / 16.
+template <bool kBf16, int K, int N, int KA, int kS0 = 0, int kS1 = K / 16>
 __device__ __forceinline__ void issue_layer(uint32_t d_tmem, uint32_t a_tmem, uint32_t one_tmem, uint32_t w_saddr, uint32_t bar)
 {
     constexpr uint32_t idesc = make_idesc<kBf16>(N);
     tc_fence_after();
 #pragma unroll
-    for (int s = 0; s < K / 16; ++s) {
+    for (int s = kS0; s < kS1; ++s) {
         const uint32_t b = w_saddr + (uint32_t)(s >> 2) * (uint32_t)N * 128u + (uint32_t)(s & 3) * 32u;
         const uint32_t a = s < KA / 16 ? a_tmem + (uint32_t)s * 8u : one_tmem + (uint32_t)(s - KA / 16) * 8u;
         umma_ts(d_tmem, a, make_b_desc(b), idesc, s > 0 ? 1u : 0u);
     }
-    umma_commit(bar);
+    if (kS1 == K / 16) umma_commit(bar);
 }
 
 

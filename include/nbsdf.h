@@ -161,14 +161,15 @@ int nbsdf_encode_latent(nbsdf_ctx* ctx, int32_t row, const float* feature_host, 
 /* Batched decoder inference: stages A1-A4, B1-B7 of DESIGN.md in one fused kernel.
  * q_dev: DEVICE, n records, 16-byte aligned.  frames_dev: DEVICE [n][6] = (normal, tangent hint) per query in
  * the space of wi/wo, or NULL when wi/wo are already local.  rgb_dev: DEVICE [n][3] fp32, 16-byte aligned.
- * n == 0 is a no-op returning NBSDF_OK; n >= 2^38 per call is NBSDF_E_INVALID (tile indices are 32-bit). */
+ * n == 0 is a no-op returning NBSDF_OK; n >= 2^37 per call is NBSDF_E_INVALID (tile indices are 32-bit and
+ * the kernels look three rounds of tiles ahead). */
 int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float* frames_dev, int64_t n, float* rgb_dev,
                void* cuda_stream);
 
 /* Frame shading: per pixel, MLP-A once, MLP-B once per light,
  * radiance[p] = sum_l rgb(z_m, uv, fp, wi_l, wo) * E_l * max(0, wi_l,local.z), lights in index order.
  * gbuf: HOST struct holding DEVICE plane pointers.  lights_host: HOST, n_lights <= NBSDF_MAX_LIGHTS, copied.
- * radiance_dev: DEVICE [h][w][3] fp32, 16-byte aligned.  width * height >= 2^38 => NBSDF_E_INVALID. */
+ * radiance_dev: DEVICE [h][w][3] fp32, 16-byte aligned.  width * height >= 2^37 => NBSDF_E_INVALID. */
 int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* gbuf, const nbsdf_light* lights_host, int32_t n_lights,
                       float* radiance_dev, void* cuda_stream);
 

@@ -478,7 +478,7 @@ extern "C" int nbsdf_eval(nbsdf_ctx* ctx, const nbsdf_query* q_dev, const float*
 {
     if (!ctx) return NBSDF_E_INVALID;
     if (n < 0) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: negative n");
-    if (n >= ((int64_t)1 << 38)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: n must be below 2^38 per call");
+    if (n >= ((int64_t)1 << 37)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: n must be below 2^37 per call");
     if (n == 0) return NBSDF_OK;
     if (!q_dev || !rgb_dev) return fail(ctx, NBSDF_E_INVALID, "nbsdf_eval: NULL buffer");
     if (!aligned16(q_dev) || !aligned16(rgb_dev) || (frames_dev && (reinterpret_cast<uintptr_t>(frames_dev) & 7u)))
@@ -506,7 +506,7 @@ extern "C" int nbsdf_shade_frame(nbsdf_ctx* ctx, const nbsdf_gbuffer* g, const n
     if (n_lights > 0 && !lights_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL lights");
     const int64_t npx = (int64_t)g->width * g->height;
     if (npx == 0) return NBSDF_OK;
-    if (npx >= ((int64_t)1 << 38)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: width * height must be below 2^38");
+    if (npx >= ((int64_t)1 << 37)) return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: width * height must be below 2^37");
     if (!g->pos_fp || !g->nrm_u || !g->tan_v || !g->material || !radiance_dev)
         return fail(ctx, NBSDF_E_INVALID, "nbsdf_shade_frame: NULL buffer");
     if (!aligned16(g->pos_fp) || !aligned16(g->nrm_u) || !aligned16(g->tan_v) || !aligned16(radiance_dev) || !aligned16(g->albedo))

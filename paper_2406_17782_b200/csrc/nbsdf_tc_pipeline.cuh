@@ -74,7 +74,8 @@ struct Pipe {
     const uint8_t* my_stage_g;
     // tensor memory
     uint32_t tmem_base, col0, lane_off, lane_taddr;
-    // tiles: indices are 32-bit (the host rejects n >= 2^38); only addresses are formed in 64 bits
+    // tiles: indices are 32-bit; the host rejects n >= 2^37, so that tile + 3 * stride (< 2^30 + 3 * 148 * 6) cannot wrap;
+    // only addresses are formed in 64 bits
     int n_tiles, n_full, last_rows, stride, first;
     const nbsdf_query* q;
     const float* frames;

@@ -318,7 +318,7 @@ def test_error_codes_and_no_fallback(cfg0):
     assert e.value.status == api.NBSDF_E_INVALID
     qd = api.queries_to_device(cfg0["queries"][:8])
     with pytest.raises(api.NbsdfError) as e:
-        api.nbsdf_eval(c.ctx, qd, None, 1 << 38, out)                     # beyond the 32-bit tile index range
+        api.nbsdf_eval(c.ctx, qd, None, 1 << 37, out)                     # beyond the 32-bit tile index range
     assert e.value.status == api.NBSDF_E_INVALID
     with pytest.raises(api.NbsdfError) as e:
         api.nbsdf_eval(c.ctx, qd[4:], None, 4, out)                      # misaligned

@@ -41,6 +41,7 @@ PD_FLOP_PER_QUERY = PD_FLOP_FUSION + PD_FLOP_ANGULAR                            
 BYTES_PER_QUERY = 40 + 12
 N_ROTATE = 8            # distinct resident batches cycled through so that no step finds its input in L2
 ROUNDS = 7              # timed rounds of `steps` launches; the median round is reported
+WORKLOAD = "configs[1]: batch eval, 2^20 queries/step/GPU, 8 materials, L=16, H=64, F=32, bf16-stored weights, fp32 I/O"
 METRIC = "decoder_bsdf_queries_per_sec"
 UNIT = "queries/s"
 # fp32 CUDA-core variant: "alu" roofline = 148 SMs x 128 FMA lanes x 2 FLOP x SM clock (guide: 148 SMs, 4 x 32 fp32
@@ -153,9 +154,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[1]: batch eval, 2^20 queries/step, 8 materials, L=16, H=64, F=32, bf16-stored "
-                                   "weights, fp32 I/O" + ("" if n_step == n_full else " (bounded sample per step)"),
-                       "queries_per_step": n_step, "latent_dim": 16, "hidden": 64, "materials": 8},
+            "config": {"workload": WORKLOAD + ("" if n_step == n_full else " (bounded sample per step)"),
+                       "queries_per_step_per_gpu": n_step, "precision": "f64 (oracle)", "latent_dim": 16, "hidden": 64,
+                       "materials": 8},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -454,8 +455,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {"fp16": "f16", "bf16": "bf16", "fp32": "f32"}[prec], "data": "synthetic",
-            "config": {"workload": "configs[1]: batch eval, 2^20 queries/step/GPU, 8 materials, L=16, H=64, F=32, "
-                                   "bf16-stored weights, fp32 I/O", "queries_per_step_per_gpu": n, "precision": prec,
+            "config": {"workload": WORKLOAD, "queries_per_step_per_gpu": n, "precision": prec,
                        "l2": f"inputs rotate over {N_ROTATE} distinct resident batches "
                              f"({N_ROTATE * n * BYTES_PER_QUERY / 1e6:.0f} MB > 126 MB L2), no flush kernel",
                        "parallelism": f"replicated weights, {world} independent query shards",

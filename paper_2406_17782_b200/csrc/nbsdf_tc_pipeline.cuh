@@ -151,8 +151,10 @@ struct Pipe {
         n_tiles = (int)((n_items + 127) / 128);
         n_full = (int)(n_items / 128);                                 // tiles [0, n_full) are complete
         last_rows = (int)(n_items - (int64_t)n_full * 128);            // live rows of the ragged tile n_full, if any
+        // tile slots in warpgroup-major order (slot = wg * grid + cta): every SM gets the same number of tiles +- 1, and a
+        // batch of fewer tiles than slots spreads over all SMs with one warpgroup each instead of filling a few CTAs
         stride = (int)gridDim.x * NWG;
-        first = (int)blockIdx.x * NWG + wg;
+        first = wg * (int)gridDim.x + (int)blockIdx.x;
         q = q_;
         frames = frames_;
         // per-query frames ride in the same staging buffer when their address allows bulk copies (16-byte aligned)
@@ -309,7 +311,7 @@ template <int NWG, typename Kern, typename... Args>
 static cudaError_t launch_persistent(Kern kern, uint32_t smem_bytes, int num_sms, int64_t n_items, cudaStream_t s, Args... args)
 {
     const int64_t tiles = (n_items + 127) / 128;
-    int64_t grid = (tiles + NWG - 1) / NWG;
+    int64_t grid = tiles;                    // one CTA per SM; fewer only when there are fewer tiles than SMs
     if (grid > num_sms) grid = num_sms;
     if (grid < 1) grid = 1;
     cudaLaunchConfig_t cfg{};

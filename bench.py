@@ -589,7 +589,7 @@ def respawn_under_torchrun(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--rounds", type=int, default=ROUNDS, help="timed rounds of --steps launches; the median is reported")
     ap.add_argument("--precision", default="fp16", choices=["fp16", "bf16", "fp32"])

@@ -158,6 +158,33 @@ int nbsdf_set_encoder(nbsdf_ctx* ctx, const nbsdf_encoder_weights* weights);
  * been installed or row is out of range. */
 int nbsdf_encode_latent(nbsdf_ctx* ctx, int32_t row, const float* feature_host, float alpha, float beta, void* cuda_stream);
 
+/* The encoder tail for callers that cannot allocate device memory -- a renderer whose own pool already holds the whole
+ * GPU, or a frame loop that cannot take the device-wide synchronisation cudaMalloc / cudaFree imply.  (The two calls
+ * above allocate: weight blob, staging slots, pinned ring.)  This call allocates NOTHING, on the device or the host, and
+ * needs no context: same arithmetic as nbsdf_encode_latent (fp32, leaky-ReLU slope 0.01), run as one small kernel per
+ * layer (4 launches) enqueued on cuda_stream of `device`; the caller's current device is restored on return.
+ *   weights_dev: HOST struct whose W[] / b[] are DEVICE pointers, fp32, row-major [out][in], shapes as listed above
+ *                with L = latent_dim; read in place (no packed copy), so they must stay valid until the work has run.
+ *   feature_dev: DEVICE, Fr fp32 (may be NULL when Fr == 0).   z_dev: DEVICE, latent_dim fp32, receives z -- e.g. the
+ *                caller's own latent buffer; to put it into a context's table copy it to the host for nbsdf_set_latents.
+ * Scratch: the activations between the launches live in ONE fixed 3-KB array inside the library image (a static
+ * __device__ array: every GPU that loads the library holds it until the process exits).  Hence
+ *   - limits: hidden <= 256 (any value, not only the four above), feat_width <= 1022, latent_dim <= 64; beyond them
+ *     the call returns NBSDF_E_UNSUPPORTED and launches nothing;
+ *   - every call on a GPU shares the array.  Calls on one stream are ordered and safe; calls that can overlap on the
+ *     GPU (two streams with no event between them, two threads) race on it and give wrong latents.  Nothing in it needs
+ *     clearing between calls: each launch reads only what an earlier launch of the same call wrote;
+ *   - the FIRST call on each device also looks up the array's device address (cudaGetSymbolAddress) and caches it:
+ *     make that call during set-up, before any stream capture.
+ * Errors: as everywhere; the text is at nbsdf_last_error(NULL). */
+int nbsdf_encode_latent_static(int32_t device, const nbsdf_encoder_weights* weights_dev, int32_t latent_dim,
+                               const float* feature_dev, float alpha, float beta, float* z_dev, void* cuda_stream);
+
+/* Reads rows [first, first+count) of the latent table back: latents_host: HOST, count x L fp32.  Enqueued on cuda_stream
+ * after the edits already queued there; BLOCKS until that copy has finished (a debugging / checking call, not part of
+ * the frame loop).  Rows out of range => NBSDF_E_INVALID. */
+int nbsdf_get_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, float* latents_host, void* cuda_stream);
+
 /* Batched decoder inference: stages A1-A4, B1-B7 of DESIGN.md in one fused kernel.
  * q_dev: DEVICE, n records, 16-byte aligned.  frames_dev: DEVICE [n][6] = (normal, tangent hint) per query in
  * the space of wi/wo, or NULL when wi/wo are already local.  rgb_dev: DEVICE [n][3] fp32, 16-byte aligned.

@@ -16,7 +16,7 @@ PRECISIONS = {"fp32": NBSDF_PREC_FP32, "bf16": NBSDF_PREC_BF16, "fp16": NBSDF_PR
 NBSDF_MAX_LIGHTS = 32
 EXPORTS = ["nbsdf_create", "nbsdf_set_latents", "nbsdf_eval", "nbsdf_shade_frame", "nbsdf_destroy",
            "nbsdf_last_error", "nbsdf_launch_count", "nbsdf_create_paper", "nbsdf_set_albedos", "nbsdf_lerp_latents",
-           "nbsdf_set_encoder", "nbsdf_encode_latent"]
+           "nbsdf_set_encoder", "nbsdf_encode_latent", "nbsdf_encode_latent_static", "nbsdf_get_latents"]
 
 
 class NbsdfError(RuntimeError):
@@ -80,6 +80,11 @@ def load():
         lib.nbsdf_set_encoder.argtypes = [C.c_void_p, C.POINTER(_EncoderWeights)]
         lib.nbsdf_encode_latent.restype = C.c_int
         lib.nbsdf_encode_latent.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
+        lib.nbsdf_encode_latent_static.restype = C.c_int
+        lib.nbsdf_encode_latent_static.argtypes = [C.c_int32, C.POINTER(_EncoderWeights), C.c_int32, C.c_void_p, C.c_float,
+                                                   C.c_float, C.c_void_p, C.c_void_p]
+        lib.nbsdf_get_latents.restype = C.c_int
+        lib.nbsdf_get_latents.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         _lib = lib
     return _lib
 
@@ -164,6 +169,32 @@ def nbsdf_encode_latent(ctx, row, feature_host, alpha, beta, stream=None):
     f = np.ascontiguousarray(feature_host, dtype=np.float32).reshape(-1)
     _check(load().nbsdf_encode_latent(ctx, int(row), f.ctypes.data if f.size else None, float(alpha), float(beta),
                                       _stream(stream)), ctx)
+
+
+def nbsdf_encode_latent_static(weights_dev, biases_dev, feature_dev, alpha, beta, z_dev, device=0, stream=None):
+    """The encoder tail without any allocation (include/nbsdf.h): for callers that cannot cudaMalloc.  weights_dev /
+    biases_dev: 4 contiguous CUDA float32 tensors each, E0 [He][Fr+2], E1, E2 [He][He], E3 [L][He], read in place;
+    feature_dev: CUDA float32 [Fr] (None when Fr == 0); z_dev: CUDA float32 [L], receives the latent.  Shapes are only
+    read off the tensors here; the size limits (He <= 256, Fr <= 1022, L <= 64) are the library's to enforce."""
+    if len(weights_dev) != 4 or len(biases_dev) != 4:
+        raise ValueError("encoder tail: 4 layers")
+    He, Fr, L = weights_dev[0].shape[0], weights_dev[0].shape[1] - 2, weights_dev[3].shape[0]
+    for w, b, s in zip(weights_dev, biases_dev, [(He, Fr + 2), (He, He), (He, He), (L, He)]):
+        if tuple(w.shape) != s or b.numel() != s[0] or not (w.is_cuda and b.is_cuda and w.is_contiguous() and b.is_contiguous()):
+            raise ValueError(f"layer {tuple(w.shape)}/{tuple(b.shape)}: expected contiguous CUDA tensors of shape {s}")
+    if z_dev.numel() != L or (Fr and (feature_dev is None or feature_dev.numel() != Fr)):
+        raise ValueError("feature must hold Fr floats and z_dev L floats")
+    ew = _EncoderWeights((C.c_void_p * 4)(*[w.data_ptr() for w in weights_dev]),
+                         (C.c_void_p * 4)(*[b.data_ptr() for b in biases_dev]), Fr, He)
+    _check(load().nbsdf_encode_latent_static(int(device), C.byref(ew), L, _ptr(feature_dev) if Fr else None, float(alpha),
+                                             float(beta), _ptr(z_dev), _stream(stream)), None)
+
+
+def nbsdf_get_latents(ctx, first, count, latent_dim, stream=None):
+    """Rows [first, first+count) of the context's latent table as a host float32 array [count][latent_dim] (blocks)."""
+    out = np.empty((count, latent_dim), dtype=np.float32)
+    _check(load().nbsdf_get_latents(ctx, int(first), int(count), out.ctypes.data, _stream(stream)), ctx)
+    return out
 
 
 def nbsdf_lerp_latents(ctx, dst, a, b, t, stream=None):

@@ -6,7 +6,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libnbsdf.so")
 LIB_PROBE = os.path.join(_HERE, "libnbsdf_probe.so")      # debug build with -DNBSDF_PROBE (csrc/nbsdf_probe.cuh); never loaded by default
-SOURCES = ["nbsdf_host.cu", "nbsdf_fp32.cu", "nbsdf_encoder.cu", "nbsdf_tc.cu", "nbsdf_tc_paper.cu"]
+SOURCES = ["nbsdf_host.cu", "nbsdf_fp32.cu", "nbsdf_encoder.cu", "nbsdf_encoder_static.cu", "nbsdf_tc.cu", "nbsdf_tc_paper.cu"]
 HEADERS = ["nbsdf_common.cuh", "nbsdf_tc_ptx.cuh", "nbsdf_tc_pipeline.cuh", "nbsdf_probe.cuh", os.path.join("..", "..", "include", "nbsdf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--threads", "0"]

@@ -48,6 +48,9 @@ struct nbsdf_ctx {
 
 static thread_local std::string g_create_err;
 
+// calls that have no context (nbsdf_encode_latent_static) report through nbsdf_last_error(NULL) as nbsdf_create does
+namespace nbsdf { void set_global_error(const char* msg) { g_create_err = msg; } }
+
 static int fail(nbsdf_ctx* ctx, int code, const std::string& msg)
 {
     if (ctx) ctx->err = msg; else g_create_err = msg;
@@ -386,6 +389,24 @@ extern "C" int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, c
     if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
     const cudaError_t e = ring_upload(ctx, ctx->d_latents + (size_t)first * L, latents_host, (size_t)count * L, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_set_latents upload", e);
+    return NBSDF_OK;
+}
+
+extern "C" int nbsdf_get_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, float* latents_host, void* cuda_stream)
+{
+    if (!ctx) return NBSDF_E_INVALID;
+    if (first < 0 || count < 0 || (int64_t)first + count > ctx->cfg.max_materials)
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_get_latents: rows out of range");
+    if (count == 0) return NBSDF_OK;
+    if (!latents_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_get_latents: NULL latents");
+    const int L = ctx->cfg.latent_dim;
+    DeviceGuard guard(ctx->cfg.device);
+    if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMemcpyAsync(latents_host, ctx->d_latents + (size_t)first * L, (size_t)count * L * sizeof(float),
+                                    cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_get_latents copy", e);
     return NBSDF_OK;
 }
 

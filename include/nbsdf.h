@@ -18,9 +18,16 @@
  *     latent table and light staging, all released by nbsdf_destroy.  HOST arrays handed to
  *     nbsdf_create / nbsdf_set_latents / nbsdf_shade_frame(lights) are copied before the call returns.
  *   - nbsdf_eval / nbsdf_shade_frame / nbsdf_set_latents / nbsdf_set_albedos / nbsdf_lerp_latents only enqueue work
- *     on the given stream and return; there is no internal synchronisation.  (Host rows handed to the two set_* calls
- *     are staged in a ring of 8 pinned slots: only a 9th edit issued while the first is still in flight waits for that
- *     one copy.)  Work is ordered by the stream: a set_latents is visible to every later launch on the same stream
+ *     on the given stream and return.  The one exception: host rows handed to nbsdf_set_latents / nbsdf_set_albedos /
+ *     nbsdf_encode_latent are staged in a ring of 8 pinned slots, and a 9th edit issued while the 1st is still
+ *     outstanding BLOCKS THE HOST until the stream has reached the 1st edit -- the copy is stream-ordered, so that means
+ *     until every kernel queued ahead of it has finished.  Up to 8 outstanding edits never block.
+ *   - A context is NOT thread-safe: its staging ring, launch counter and error text are plain members.  Use one context
+ *     per host thread, or serialise the calls on a context yourself.  Different contexts are independent.
+ *   - CUDA graphs: nbsdf_eval / nbsdf_shade_frame / nbsdf_lerp_latents may be captured.  nbsdf_set_latents /
+ *     nbsdf_set_albedos / nbsdf_encode_latent return NBSDF_E_INVALID on a capturing stream and enqueue nothing (a replay
+ *     would re-read a pinned slot the host has reused): issue edits between replays.
+ *   - Work is ordered by the stream: a set_latents is visible to every later launch on the same stream
  *     (the editing guarantee of PAPER.md:198).  Every call works on cfg.device and restores the caller's current
  *     CUDA device before it returns.
  *   - Every call returns an nbsdf_status and never throws or aborts; nbsdf_last_error gives text.
@@ -33,9 +40,9 @@
  *     never a fault.
  *   - Operand precision: NBSDF_PREC_FP16 (the default of the Python binding) meets max 1e-2 / mean 2e-3 against the
  *     fp64 definition on every supported dims with ~8x margin.  NBSDF_PREC_BF16 exists for networks whose activations
- *     exceed the fp16 range; its 8-bit significands meet the mean bound everywhere but the max bound only with < 2x
- *     margin (measured 0.35e-2 .. 1.14e-2 over the supported dims) -- use fp16 where the bound
- *     must hold.
+ *     exceed the fp16 range; its 8-bit significands cannot hold the max bound for hidden = 32 (any latent_dim) or for
+ *     (latent_dim 32, hidden 64) (0.5e-2 .. 1.2e-2), and nbsdf_create REJECTS bf16 there with
+ *     NBSDF_E_UNSUPPORTED rather than serve it at a looser tolerance; at the remaining dims the five-seed emulation stays <= 0.8e-2.
  */
 #ifndef NBSDF_H
 #define NBSDF_H

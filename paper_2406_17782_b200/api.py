@@ -54,8 +54,7 @@ def load():
     """Build (if stale) and dlopen libnbsdf.so; declare the prototypes of include/nbsdf.h."""
     global _lib
     if _lib is None:
-        import os
-        lib = C.CDLL(os.environ.get("NBSDF_LIB") or buildlib.build())      # NBSDF_LIB: probe.py's instrumented debug build
+        lib = C.CDLL(buildlib.build())
         lib.nbsdf_create.restype = C.c_int
         lib.nbsdf_create.argtypes = [C.POINTER(_Config), C.POINTER(_Weights), C.POINTER(C.c_void_p)]
         lib.nbsdf_set_latents.restype = C.c_int

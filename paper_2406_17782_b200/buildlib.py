@@ -5,9 +5,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libnbsdf.so")
-LIB_PROBE = os.path.join(_HERE, "libnbsdf_probe.so")      # debug build with -DNBSDF_PROBE (csrc/nbsdf_probe.cuh); never loaded by default
 SOURCES = ["nbsdf_host.cu", "nbsdf_fp32.cu", "nbsdf_encoder.cu", "nbsdf_encoder_static.cu", "nbsdf_tc.cu", "nbsdf_tc_paper.cu"]
-HEADERS = ["nbsdf_common.cuh", "nbsdf_tc_ptx.cuh", "nbsdf_tc_pipeline.cuh", "nbsdf_probe.cuh", os.path.join("..", "..", "include", "nbsdf.h")]
+HEADERS = ["nbsdf_common.cuh", "nbsdf_tc_ptx.cuh", "nbsdf_tc_pipeline.cuh", os.path.join("..", "..", "include", "nbsdf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--threads", "0"]
 
@@ -27,19 +26,18 @@ def _stale(lib):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False, probe=False):
-    """Compile csrc/*.cu into libnbsdf.so (one object per source, in parallel) and return its path.
-    probe=True builds the instrumented debug library libnbsdf_probe.so instead (used only by probe.py)."""
-    lib = LIB_PROBE if probe else LIB
+def build(force=False, verbose=False):
+    """Compile csrc/*.cu into libnbsdf.so (one object per source, in parallel) and return its path."""
+    lib = LIB
     if not (force or _stale(lib)):
         return lib
     objs, procs = [], []
-    bdir = os.path.join(_HERE, "build", "probe" if probe else "")
+    bdir = os.path.join(_HERE, "build")
     os.makedirs(bdir, exist_ok=True)
     for s in SOURCES:
         o = os.path.join(bdir, s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-DNBSDF_PROBE"] if probe else []) + os.environ.get("NBSDF_EXTRA_NVCC", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
+        cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("NBSDF_EXTRA_NVCC", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, p in procs:
         out, _ = p.communicate()
@@ -53,4 +51,4 @@ def build(force=False, verbose=False, probe=False):
 
 if __name__ == "__main__":
     import sys
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, probe="--probe" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

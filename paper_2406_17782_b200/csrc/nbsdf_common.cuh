@@ -19,13 +19,17 @@ struct NetParams {
     const uint8_t* wimg_shade;   // tensor path: shared-memory image for nbsdf_shade_frame (6 layers)
     const float* albedos;        // paper-structured decoder: [M][12] fp32 (kd_warp, kd_weft, ks_warp, ks_weft) x RGB
     int32_t L, H, M;
-#ifdef NBSDF_PROBE
-    int32_t probe_slot;          // debug builds only (nbsdf_probe.cuh): launch counter of the context
-#endif
 };
 
 struct LightParams {
     nbsdf_light light[NBSDF_MAX_LIGHTS];   // directional vec already normalised on the host
+    int32_t n;
+};
+
+// What an EVAL launch passes in place of the 1.3-KB light table it never reads (kernel parameters are copied at every
+// launch: at 2^12..2^16 queries the launch is latency-bound and the parameter block is part of that latency).
+struct NoLightParams {
+    nbsdf_light light[1];
     int32_t n;
 };
 

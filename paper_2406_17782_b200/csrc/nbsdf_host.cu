@@ -84,6 +84,14 @@ static cudaError_t ring_create(nbsdf_ctx* ctx, size_t slot_floats)
 }
 
 // host rows -> next pinned slot -> cudaMemcpyAsync to dst on stream s; never waits unless the ring has wrapped
+// The pinned ring cannot live inside a CUDA graph: a captured copy would re-read, on every replay, a slot the host has
+// long since reused, and the slot's event would be captured instead of recorded.  Edits go between replays.
+static bool stream_is_capturing(cudaStream_t s)
+{
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    return cudaStreamIsCapturing(s, &st) == cudaSuccess && st != cudaStreamCaptureStatusNone;
+}
+
 static cudaError_t ring_upload(nbsdf_ctx* ctx, float* dst, const float* src_host, size_t n_floats, cudaStream_t s,
                                const float* tail = nullptr, size_t n_tail = 0, float* dst_slots = nullptr, size_t dst_stride = 0,
                                int* slot_out = nullptr)
@@ -191,6 +199,13 @@ extern "C" int nbsdf_create(const nbsdf_config* cfg, const nbsdf_weights* weight
     if (!dims_supported(cfg))
         return fail(nullptr, NBSDF_E_UNSUPPORTED,
                     "nbsdf_create: supported dims are latent_dim in {8,16,32}, hidden in {32,64,128}, feat_dim 32, 1..64 materials");
+    // bf16 operands are served only where they meet the stated bound (max 1e-2 / mean 2e-3) with margin: the 8-bit
+    // significands of the hidden activations put the max at 0.5-1.2e-2 for every H = 32 network and at 1.1e-2 for
+    // (L 32, H 64) (tests/quant_emulation.py, no GPU involved) -- rejected, as nbsdf_create_paper does
+    if (cfg->precision == NBSDF_PREC_BF16 && (cfg->hidden == 32 || (cfg->latent_dim == 32 && cfg->hidden == 64)))
+        return fail(nullptr, NBSDF_E_UNSUPPORTED,
+                    "nbsdf_create: bf16 operands cannot meet the 1e-2 max bound at hidden 32 or at (latent_dim 32, hidden 64); "
+                    "use NBSDF_PREC_FP16 there");
     int n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
     if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceCount", e);
@@ -345,6 +360,9 @@ extern "C" int nbsdf_set_albedos(nbsdf_ctx* ctx, int32_t first, int32_t count, c
     if (!albedos_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: NULL albedos");
     DeviceGuard guard(ctx->cfg.device);
     if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    if (stream_is_capturing((cudaStream_t)cuda_stream))
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_albedos: the stream is being captured; host edits cannot be part of a CUDA graph "
+                                          "(issue them between replays)");
     const cudaError_t e = ring_upload(ctx, ctx->d_albedos + (size_t)first * 12, albedos_host, (size_t)count * 12, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_set_albedos upload", e);
     return NBSDF_OK;
@@ -387,6 +405,9 @@ extern "C" int nbsdf_set_latents(nbsdf_ctx* ctx, int32_t first, int32_t count, c
     const int L = ctx->cfg.latent_dim;
     DeviceGuard guard(ctx->cfg.device);
     if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    if (stream_is_capturing((cudaStream_t)cuda_stream))
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_set_latents: the stream is being captured; host edits cannot be part of a CUDA graph "
+                                          "(issue them between replays)");
     const cudaError_t e = ring_upload(ctx, ctx->d_latents + (size_t)first * L, latents_host, (size_t)count * L, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_set_latents upload", e);
     return NBSDF_OK;
@@ -447,6 +468,9 @@ extern "C" int nbsdf_encode_latent(nbsdf_ctx* ctx, int32_t row, const float* fea
     if (ctx->enc_fr > 0 && !feature_host) return fail(ctx, NBSDF_E_INVALID, "nbsdf_encode_latent: NULL feature");
     DeviceGuard guard(ctx->cfg.device);
     if (guard.err != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", guard.err);
+    if (stream_is_capturing((cudaStream_t)cuda_stream))
+        return fail(ctx, NBSDF_E_INVALID, "nbsdf_encode_latent: the stream is being captured; host edits cannot be part of a CUDA graph "
+                                          "(issue them between replays)");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const float ab[2] = { alpha, beta };
     int slot = 0;
@@ -456,6 +480,10 @@ extern "C" int nbsdf_encode_latent(nbsdf_ctx* ctx, int32_t row, const float* fea
     e = launch_encode_latent(ctx->d_enc_w, ctx->d_enc_in + (size_t)slot * nbsdf_ctx::kEncInFloats, ctx->enc_fr, ctx->enc_he, L,
                              ctx->d_latents + (size_t)row * L, s);
     if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_encode_latent launch", e);
+    // the slot (pinned AND device side) is free only when the kernel that reads it has run, not when the copy has:
+    // re-record the slot's event behind the launch, so that a wrapped ring waits for the reader even across streams
+    e = cudaEventRecord(ctx->ring_ev[slot], s);
+    if (e != cudaSuccess) return fail_cuda(ctx, "nbsdf_encode_latent event", e);
     ctx->launches += 1;
     return NBSDF_OK;
 }
@@ -486,9 +514,6 @@ static NetParams net_params(const nbsdf_ctx* ctx)
     p.L = ctx->cfg.latent_dim;
     p.H = ctx->cfg.hidden;
     p.M = ctx->cfg.max_materials;
-#ifdef NBSDF_PROBE
-    p.probe_slot = (int32_t)ctx->launches;
-#endif
     return p;
 }
 

@@ -18,6 +18,8 @@
 //   [0, H)              accumulator
 //   [H, H + H/2)        AH: z at the start of a tile, then the hidden activations
 //   [H + H/2, +24)      AY: [blob(24), c] for round 1 (16 columns), then y = [feat(32), wi(3), wo(2), c] (20 of 24 columns)
+#include <type_traits>
+
 #include "nbsdf_tc_pipeline.cuh"
 
 namespace nbsdf {
@@ -115,7 +117,7 @@ __device__ __forceinline__ float fast_expm1(float y)
 template <int H, int NWG, bool kShade>
 __global__ void __launch_bounds__(Pd<H, NWG, kShade>::kThreads, 1)
 pd_kernel(NetParams net, const nbsdf_query* __restrict__ q, const float* __restrict__ frames, int64_t n,
-          FrameParams fr, LightParams lights, float* __restrict__ out)
+          FrameParams fr, std::conditional_t<kShade, LightParams, NoLightParams> lights, float* __restrict__ out)
 {
     using T = Pd<H, NWG, kShade>;
     constexpr int L = kPdLatent;
@@ -445,7 +447,12 @@ static cudaError_t pd_dispatch(const NetParams& net, int num_sms, const nbsdf_qu
     using T = Pd<64, NWG, kShade>;
     auto kern = pd_kernel<64, NWG, kShade>;
     if (init_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::smem_bytes());
-    return launch_persistent<NWG>(kern, T::smem_bytes(), num_sms, kShade ? fr.n_pixels : n, s, net, q, frames, n, fr, lights, out);
+    if constexpr (kShade) {
+        return launch_persistent<NWG>(kern, T::smem_bytes(), num_sms, fr.n_pixels, s, net, q, frames, n, fr, lights, out);
+    } else {
+        NoLightParams none{};
+        return launch_persistent<NWG>(kern, T::smem_bytes(), num_sms, n, s, net, q, frames, n, fr, none, out);
+    }
 }
 
 cudaError_t init_pd(int H)

@@ -10,7 +10,7 @@ while accumulation, biases and the output activation stay exact, as they do in a
 With identity hooks it must reproduce the C oracle (asserted on every run), so every number it prints is "oracle with
 the named operands rounded".  It calls only oracle/ and the seeded input generator.
 
-    python oracle/quant_study.py [--n 65536] [--md]      # prints the table of BASELINE.md sec. 5
+    python tests/quant_emulation.py [--n 65536] [--md]      # prints the table of BASELINE.md sec. 5
 
 Formats: fp16 (11-bit significand), bf16 (8), e4m3 (4; max 448, subnormals down to 2^-9, saturating) with a per-layer
 power-of-two scale chosen from the layer's own max magnitude (the best case for a per-layer-scaled FP8 kernel), e5m2 (3).

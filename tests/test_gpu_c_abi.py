@@ -65,6 +65,44 @@ def test_eval_inside_a_cuda_graph_and_latent_edit_between_replays():
     api.nbsdf_destroy(ctx)
 
 
+def test_host_edits_are_refused_on_a_capturing_stream():
+    """include/nbsdf.h: the pinned staging ring cannot be replayed, so set_latents / set_albedos / encode_latent return
+    NBSDF_E_INVALID while the stream is being captured and enqueue nothing; the capture itself stays valid."""
+    cfg = synth.config(1, n=4096)
+    enc = synth.enc_config(feat_width=32, hidden=64, latent=16)
+    ctx = api.nbsdf_create(cfg["weights"], cfg["biases"], 16, 64, 8, "fp16")
+    api.nbsdf_set_latents(ctx, 0, cfg["latents"])
+    api.nbsdf_set_encoder(ctx, enc["weights"], enc["biases"])
+    pd = synth.pd_config("eval", n=8)
+    pctx = api.nbsdf_create_paper(pd["weights"], pd["biases"], 64, 8, "fp16")
+    n = len(cfg["queries"])
+    qd = api.queries_to_device(cfg["queries"])
+    out = torch.zeros((n, 3), dtype=torch.float32, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        api.nbsdf_eval(ctx, qd, None, n, out)
+    torch.cuda.current_stream().wait_stream(side)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for call in (lambda: api.nbsdf_set_latents(ctx, 2, np.full(16, 9.0, np.float32)),
+                     lambda: api.nbsdf_encode_latent(ctx, 2, enc["features"][0], 0.5, 1.0),
+                     lambda: api.nbsdf_set_albedos(pctx, 0, pd["albedos"])):
+            with pytest.raises(api.NbsdfError) as e:
+                call()
+            assert e.value.status == api.NBSDF_E_INVALID and "captured" in str(e.value)
+        api.nbsdf_eval(ctx, qd, None, n, out)
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"])     # row 2 was NOT edited
+    check(out.cpu().numpy(), ref, "fp16", "replay after refused edits")
+    api.nbsdf_set_latents(ctx, 2, cfg["latents"][2])                                                # and works again outside
+    torch.cuda.synchronize()
+    api.nbsdf_destroy(ctx)
+    api.nbsdf_destroy(pctx)
+
+
 def test_two_contexts_on_two_streams_concurrently():
     ca, cb = synth.config(1, n=200000), synth.config(4, n=150000, L=32, H=128, seed=77)
     xa = api.nbsdf_create(ca["weights"], ca["biases"], 16, 64, 8, "fp16")

@@ -31,9 +31,13 @@ def test_encode_then_eval_matches_oracle(prec, L, He, Fr):
     for m in range(8):                                        # ... and every row is then replaced by the encoder
         api.nbsdf_encode_latent(c.ctx, m, enc["features"][m], enc["alpha"][m], enc["beta"][m])
     out = c.eval(cfg["queries"])
+    z_dev = api.nbsdf_get_latents(c.ctx, 0, 8, L)                # the latent rows themselves, not only what rendering shows
     c.close()
     Z = oracle_latents(enc)
     assert np.abs(Z).max() > 0.1
+    Z64 = np.stack([oracle.encode_latent(enc["weights"], enc["biases"], enc["features"][m], enc["alpha"][m], enc["beta"][m])
+                    for m in range(8)])
+    assert np.abs(z_dev - Z64).max() <= 1e-5 * np.abs(Z64).max(), np.abs(z_dev - Z64).max()      # fp32 kernel vs fp64
     ref = oracle.eval_queries(cfg["weights"], cfg["biases"], Z, cfg["queries"])
     check(out, ref, prec, f"encode -> eval L={L} He={He} Fr={Fr}")
 
@@ -95,6 +99,7 @@ def test_encoder_errors_and_latency():
     e1.record()
     torch.cuda.synchronize()
     us = 1e3 * e0.elapsed_time(e1) / 200
-    print(f"encoder tail (Fr=256, He=128, L=16): {us:.1f} us per nbsdf_encode_latent (paper: ~0.5 ms incl. the ResNet trunk)")
-    assert us < 500.0
+    # reported only: the paper's ~0.5 ms per edit includes the ResNet-18 trunk, which is not built here
+    # (out of scope, no textures and no weights), so there is nothing to compare this tail-only figure with
+    print(f"encoder tail (Fr=256, He=128, L=16): {us:.1f} us per nbsdf_encode_latent")
     c.close()

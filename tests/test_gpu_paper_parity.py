@@ -139,6 +139,31 @@ def test_paper_frame_shading_and_albedo_edit(prec):
     c.close()
 
 
+def test_paper_decoder_with_64_materials():
+    """max_materials = 64 on the paper-structured kernel: the padded 64-row latent table and the 64 x 12 albedo table at
+    full size, per-pixel-random material ids; every output of a multi-tile batch and of a frame against the oracle."""
+    M = 64
+    cfg = synth.pd_config("eval", n=148 * 128 * 2 + 91, M=M, seed=64)
+    q = cfg["queries"]
+    q["material"][:M] = np.arange(M)
+    q["material"][M + 1::89] = -1
+    c = PCtx(cfg, "fp16", M=M)
+    out = c.eval(q)
+    fcfg = synth.pd_config("frame", width=301, height=97, M=M, seed=65)
+    g, lights = fcfg["gbuffer"], fcfg["lights"]
+    g["material"] = np.random.default_rng(66).integers(-1, M, size=301 * 97).astype(np.int32)
+    c2 = PCtx(fcfg, "fp16", M=M)
+    fr = c2.shade(g, lights)
+    c.close()
+    c2.close()
+    live = q["material"] >= 0
+    assert len(np.unique(q["material"])) == M + 1 and (out[~live] == 0).all()
+    check(out[live], oracle.pd_eval_queries(*_args(cfg), q)[live], "paper decoder, 64 materials, eval")
+    lv = g["material"] >= 0
+    assert (fr[~lv] == 0).all()
+    check(fr[lv], oracle.pd_shade_frame(*_args(fcfg), g, lights)[lv], "paper decoder, 64 materials, frame")
+
+
 def test_paper_frame_with_emitter_normals():
     """Point lights with an emitter normal (E = I max(0, -wi . n_e) / d^2), one of them behind the fabric, one facing
     away (contributes exactly 0): pd_kernel's light loop against the oracle."""

@@ -17,6 +17,11 @@ TOL = {"fp32": (1e-5, 1e-5), "bf16": (1e-2, 2e-3), "fp16": (1e-2, 2e-3)}
 PRECS = ["fp32", "fp16", "bf16"]
 
 
+def bf16_served(L, H):
+    """include/nbsdf.h: nbsdf_create rejects bf16 operands where they cannot hold the max bound (H = 32; L 32 / H 64)."""
+    return H != 32 and (L, H) != (32, 64)
+
+
 def rel_err(gpu, ref):
     gpu = np.asarray(gpu, np.float64).reshape(-1, 3)
     ref = np.asarray(ref, np.float64).reshape(-1, 3)
@@ -200,6 +205,11 @@ def test_config3_editing_small(prec):
 def test_config4_dims(prec, L, H):
     seed = synth.sweep_seed(0, [32, 64, 128].index(H), [8, 16, 32].index(L))
     cfg = synth.config(4, n=1500, L=L, H=H, seed=seed)
+    if prec == "bf16" and not bf16_served(L, H):
+        with pytest.raises(api.NbsdfError) as e:                 # not served at a private tolerance: rejected at create
+            api.nbsdf_create(cfg["weights"], cfg["biases"], L, H, 8, "bf16")
+        assert e.value.status == api.NBSDF_E_UNSUPPORTED and "bf16" in str(e.value)
+        return
     ref = oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], cfg["queries"])
     c = Ctx(cfg, prec, L=L, H=H)
     out = c.eval(cfg["queries"])
@@ -209,6 +219,43 @@ def test_config4_dims(prec, L, H):
     c.close()
     check(out, ref, prec, f"L={L} H={H}")
     check(fr, oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, lights), prec, f"frame L={L} H={H}")
+
+
+@pytest.mark.parametrize("prec", ["fp16", "fp32"])
+@pytest.mark.parametrize("L,H", [(32, 64), (32, 128), (16, 32)])
+def test_64_materials_eval_and_frame(prec, L, H):
+    """max_materials = 64, the largest latent table the boundary accepts (include/nbsdf.h; one latent per
+    fabric material of the scene): the shared-memory latent table at its full 64 x L size, material ids over the whole
+    range in every tile, every output of a multi-tile batch and of a frame against the oracle."""
+    M = 64
+    rng = np.random.default_rng(6400 + L + H)
+    cfg = synth.config(4, n=1, L=L, H=H, seed=640 + L + H)
+    cfg["latents"] = synth.make_latents(rng, M, L)
+    n = 148 * 128 + 77 if prec == "fp16" else 6000
+    q = synth.make_queries(rng, n, M)
+    q["material"][:M] = np.arange(M)                                  # every row of the table is used
+    q["material"][M + 3::101] = -1
+    frames = synth.make_frames(rng, n)
+    g = synth.make_gbuffer(rng, 333, 90)
+    g["material"] = rng.integers(-1, M, size=333 * 90).astype(np.int32)   # incoherent ids over the whole table, some background
+    assert len(np.unique(q["material"])) == M + 1 and len(np.unique(g["material"])) == M + 1
+    c = Ctx(cfg, prec, L=L, H=H, M=M)
+    out, out_f = c.eval(q), c.eval(q, frames)
+    fr = c.shade(g, synth.lights_direct5())
+    api.nbsdf_set_latents(c.ctx, M - 1, cfg["latents"][0])             # edit of the LAST row
+    out_e = c.eval(q)
+    c.close()
+    live = q["material"] >= 0
+    assert (out[~live] == 0).all()
+    check(out[live], oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], q)[live], prec, f"M=64 eval L={L} H={H}")
+    check(out_f[live], oracle.eval_queries(cfg["weights"], cfg["biases"], cfg["latents"], q, frames)[live], prec, "M=64 eval+frames")
+    lv = g["material"] >= 0
+    check(fr[lv], oracle.shade_frame(cfg["weights"], cfg["biases"], cfg["latents"], g, synth.lights_direct5())[lv], prec, "M=64 frame")
+    Z2 = cfg["latents"].copy()
+    Z2[M - 1] = Z2[0]
+    check(out_e[live], oracle.eval_queries(cfg["weights"], cfg["biases"], Z2, q)[live], prec, "M=64 after editing row 63")
+    same = live & (q["material"] != M - 1)
+    np.testing.assert_array_equal(out_e[same].view(np.uint32), out[same].view(np.uint32))
 
 
 @pytest.mark.parametrize("prec", ["fp16", "bf16"])
@@ -377,9 +424,10 @@ def test_staging_pipeline_depths(prec):
 
 
 def test_back_to_back_edits_do_not_block_and_are_ordered():
-    """Twenty set_latents calls in a row on a stream that is BUSY (a long kernel queue in front of them): the calls only
-    enqueue (ring of pinned slots; at most the wrap-around waits for one earlier copy, never for the queued kernels), each
-    host array may be overwritten as soon as its call returns, and the last edit wins for the next launch."""
+    """Twenty set_latents calls in a row on a stream that is BUSY (a long kernel queue in front of them): the first eight
+    (the ring of pinned slots) only enqueue and are timed; from the ninth on a call waits until the stream has reached the
+    edit whose slot it reuses, i.e. for the kernels queued ahead of that edit (include/nbsdf.h says so) -- those are not
+    timed.  Each host array may be overwritten as soon as its call returns, and the last edit wins for the next launch."""
     import time
     cfg = synth.config(1, n=1 << 20)
     c = Ctx(cfg, "fp16")

@@ -126,6 +126,13 @@ def oracle_rate(cfg, n_sample, threads=0, min_seconds=0.0):
             return passes * len(q) / dt, dt, passes
 
 
+def arm_config(n_step, prec, bounded=False):
+    """The `config` of BOTH arms of the bench (the driver compares them): same keys, same values for the same workload."""
+    return {"workload": WORKLOAD + (" (bounded sample per step)" if bounded else ""), "queries_per_step_per_gpu": n_step,
+            "latent_dim": 16, "hidden": 64, "materials": 8,
+            "precision": f"product arm: {prec} operands, fp32 accumulate; reference arm: the fp64 oracle"}
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, stepping over configs[1].  A step is the FULL 2^20-query batch
     when steps + warmup such steps fit the time budget (they do at the driver's 20 + 3), else a bounded sample of it."""
@@ -154,9 +161,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD + ("" if n_step == n_full else " (bounded sample per step)"),
-                       "queries_per_step_per_gpu": n_step, "precision": "f64 (oracle)", "latent_dim": 16, "hidden": 64,
-                       "materials": 8},
+            "config": arm_config(n_step, args.precision, bounded=n_step != n_full),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -192,13 +197,22 @@ def _rotations(arr, n_rot, shift):
     return [np.roll(arr, r * shift, axis=0) for r in range(n_rot)]
 
 
-def wl_eval(torch, api, synth, dev, prec, L=16, H=64, n=1 << 20, seed=None, frames=False, cfg_idx=1):
+def wl_eval(torch, api, synth, dev, prec, L=16, H=64, n=1 << 20, seed=None, frames=False, cfg_idx=1, M=8, order=None):
+    """order: None = material ids as the generator draws them (i.i.d. uniform per query: fully incoherent), "sorted" = the
+    same queries stably sorted by material id (what a sort/bin pre-pass would hand the kernel)."""
     cfg = synth.config(cfg_idx, n=n, L=L, H=H, seed=seed)
-    ctx = api.nbsdf_create(cfg["weights"], cfg["biases"], L, H, 8, prec, device=dev.index or 0)
+    if M != 8:                                      # the largest gather: a 64-row latent table, ids over the whole range
+        rng = np.random.default_rng(1000 + M)
+        cfg["latents"] = synth.make_latents(rng, M, L)
+        cfg["queries"]["material"] = rng.integers(0, M, size=n).astype(np.int32)
+    if order == "sorted":
+        cfg["queries"] = cfg["queries"][np.argsort(cfg["queries"]["material"], kind="stable")]
+    ctx = api.nbsdf_create(cfg["weights"], cfg["biases"], L, H, M, prec, device=dev.index or 0)
     api.nbsdf_set_latents(ctx, 0, cfg["latents"])
     per_q = BYTES_PER_QUERY + (24 if frames else 0)
     n_rot = N_ROTATE if n * per_q * N_ROTATE <= 3e9 else max(1, int(3e9 // (n * per_q)))
-    qs = [torch.from_numpy(q.view(np.uint8).reshape(-1).copy()).to(dev) for q in _rotations(cfg["queries"], n_rot, 12345)]
+    shift = 12345 if order is None else 0           # a rotation would split the sorted runs; distinct buffers still rotate
+    qs = [torch.from_numpy(q.view(np.uint8).reshape(-1).copy()).to(dev) for q in _rotations(cfg["queries"], n_rot, shift)]
     frs = None
     if frames:
         fr_host = synth.make_frames(np.random.default_rng(77), n)
@@ -212,8 +226,9 @@ def wl_eval(torch, api, synth, dev, prec, L=16, H=64, n=1 << 20, seed=None, fram
     return {"step": step, "ctx": ctx, "cfg": cfg, "units": n, "flop": flop * n, "bytes": per_q * n, "flop_per_unit": flop,
             "bound": "alu" if prec == "fp32" else "tensor", "q_dev": qs, "out_dev": outs, "n_rot": n_rot,
             "kernel": "eval_fp32_kernel" if prec == "fp32" else f"tc_kernel<{L},{H},{prec},eval>",
-            "workload": f"batch eval, {n} queries/launch, 8 materials, L={L}, H={H}, F=32, bf16-stored weights, fp32 I/O"
-                        + (", per-query world frame (64 B in + 12 B out)" if frames else ""),
+            "workload": f"batch eval, {n} queries/launch, {M} materials, L={L}, H={H}, F=32, bf16-stored weights, fp32 I/O"
+                        + (", per-query world frame (64 B in + 12 B out)" if frames else "")
+                        + (", queries sorted by material id" if order == "sorted" else ""),
             "close": lambda: api.nbsdf_destroy(ctx)}
 
 
@@ -286,6 +301,11 @@ CASES = {
     "eval_h32": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=16, H=32, n=1 << 22, seed=s.sweep_seed(5, 0, 1), cfg_idx=4),
     "eval_h128": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=16, H=128, n=1 << 22, seed=s.sweep_seed(5, 2, 1), cfg_idx=4),
     "eval_l32": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=32, H=64, n=1 << 20, seed=s.sweep_seed(4, 1, 2), cfg_idx=4),
+    "eval_h32_frames": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=16, H=32, n=1 << 22, seed=s.sweep_seed(5, 0, 1), cfg_idx=4, frames=True),
+    "eval_m64_l32": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=32, H=64, n=1 << 20, seed=s.sweep_seed(4, 1, 2), cfg_idx=4, M=64),
+    "eval_m64_l32_h32_frames": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=32, H=32, n=1 << 22, seed=s.sweep_seed(5, 0, 2), cfg_idx=4, M=64, frames=True),
+    "eval_sorted": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, order="sorted"),
+    "eval_m64_l32_sorted": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, L=32, H=64, n=1 << 20, seed=s.sweep_seed(4, 1, 2), cfg_idx=4, M=64, order="sorted"),
     "eval_2p24": lambda t, a, s, d, p: wl_eval(t, a, s, d, p, n=1 << 24),
     "frame": lambda t, a, s, d, p: wl_frame(t, a, s, d, p, 2),
     "frame_4k": lambda t, a, s, d, p: wl_frame(t, a, s, d, p, 3),
@@ -308,7 +328,8 @@ def measure(torch, w, steps, warmup, peaks, barrier=lambda: None, reduce_max=lam
     return {"workload": w["workload"], "kernel": w["kernel"], "ms_per_launch": med / steps, "ms_per_launch_min": lo / steps,
             "ms_per_launch_max": hi / steps, "steps": steps, "rounds": rounds, "units_per_s": w["units"] / sec,
             "flop_per_unit": w["flop_per_unit"], "achieved_tflops": tf, "bound": w["bound"], "peak_tflops": peak,
-            "frac": tf / peak, "hbm_gbs_algorithmic": w["bytes"] / sec / 1e9}
+            "frac": tf / peak, "hbm_gbs_algorithmic": w["bytes"] / sec / 1e9,
+            "hbm_frac": w["bytes"] / sec / 1e9 / peaks["hbm_gbs"], "bytes_per_unit": w["bytes"] / w["units"]}
 
 
 def run_case(args):
@@ -416,10 +437,26 @@ def run_ours(args):
     del wf
     torch.cuda.empty_cache()
 
+    # ---- the headline kernel in the SUSTAINED regime (rank 0): one ~0.25-s round of back-to-back launches, against the
+    # sustained cuBLAS peak -- burst over burst above, sustained over sustained here, never mixed ----
+    sustained = None
+    if rank == 0 and prec != "fp32":
+        k_sus = 8000
+        smp = ClockSampler(local_rank)
+        smp.start()
+        ms_sus = sorted(time_loop(torch, w["step"], k_sus, lambda: None) for _ in range(3))[1]
+        clk_sus = smp.stop()
+        tf_sus = FLOP_PER_QUERY * n * k_sus / (ms_sus * 1e-3) / 1e12
+        sustained = {"launches_per_round": k_sus, "rounds": 3, "ms_per_round": ms_sus, "queries_per_s": n * k_sus / (ms_sus * 1e-3),
+                     "achieved": tf_sus, "peak": peaks["bf16_tflops_sustained"] or None, "unit": "TFLOP/s",
+                     "frac": tf_sus / peaks["bf16_tflops_sustained"] if peaks["bf16_tflops_sustained"] else None, "clocks": clk_sus}
+
     # ---- secondary workloads, rank 0 only (not part of the scaled value) ----
     extras = {}
     if rank == 0 and prec != "fp32":
-        for key, case, k_cap in (("eval_with_frames", "eval_frames", 200), ("frame_4k", "frame_4k", 10),
+        for key, case, k_cap in (("eval_with_frames", "eval_frames", 200), ("eval_sorted_by_material", "eval_sorted", 200),
+                                 ("eval_h32_frames", "eval_h32_frames", 50), ("eval_m64_l32", "eval_m64_l32", 200),
+                                 ("eval_m64_l32_sorted", "eval_m64_l32_sorted", 200), ("frame_4k", "frame_4k", 10),
                                  ("paper_eval", "paper_eval", 200), ("paper_frame", "paper_frame", 30),
                                  ("fp32_variant", "fp32_eval", 10), ("fp32_variant_frame", "fp32_frame", 3)):
             wx = CASES[case](torch, api, synth, dev, prec)
@@ -431,7 +468,8 @@ def run_ours(args):
             torch.cuda.empty_cache()
         for key in ("frame_4k", "paper_frame", "fp32_variant_frame"):
             extras[key]["frame_ms"] = extras[key]["ms_per_launch"]
-        for key in ("eval_with_frames", "paper_eval", "fp32_variant"):
+        for key in ("eval_with_frames", "eval_sorted_by_material", "eval_h32_frames", "eval_m64_l32", "eval_m64_l32_sorted",
+                    "paper_eval", "fp32_variant"):
             extras[key]["queries_per_s"] = extras[key]["units_per_s"]
 
     line = None
@@ -455,11 +493,11 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {"fp16": "f16", "bf16": "bf16", "fp32": "f32"}[prec], "data": "synthetic",
-            "config": {"workload": WORKLOAD, "queries_per_step_per_gpu": n, "precision": prec,
-                       "l2": f"inputs rotate over {N_ROTATE} distinct resident batches "
-                             f"({N_ROTATE * n * BYTES_PER_QUERY / 1e6:.0f} MB > 126 MB L2), no flush kernel",
-                       "parallelism": f"replicated weights, {world} independent query shards",
-                       "timing": f"median of {R} rounds of {K} launches each (ms_per_step_min / _max: the fastest / slowest round)"},
+            "config": arm_config(n, prec),
+            "notes": {"l2": f"inputs rotate over {N_ROTATE} distinct resident batches "
+                            f"({N_ROTATE * n * BYTES_PER_QUERY / 1e6:.0f} MB > 126 MB L2), no flush kernel",
+                      "parallelism": f"replicated weights, {world} independent query shards",
+                      "timing": f"median of {R} rounds of {K} launches each (ms_per_step_min / _max: the fastest / slowest round)"},
             "ms_per_step_min": ms_min / K, "ms_per_step_max": ms_max / K, "rounds": R,
             "roofline": {"bound": "tensor" if prec != "fp32" else "alu", "achieved": achieved_tf,
                          "peak": peak, "unit": "TFLOP/s", "frac": achieved_tf / peak,
@@ -467,17 +505,22 @@ def run_ours(args):
                          else "148 SMs x 128 FMA lanes x 2 x 1.965 GHz",
                          "frac_of_sustained": achieved_tf / peaks["bf16_tflops_sustained"] if peaks["bf16_tflops_sustained"] and prec != "fp32" else None,
                          "kernel": w["kernel"], "us_per_launch": us_per_launch, "flop_per_query": FLOP_PER_QUERY,
-                         "hbm_gbs_algorithmic": BYTES_PER_QUERY * n / (us_per_launch * 1e-6) / 1e9},
+                         "hbm_gbs_algorithmic": BYTES_PER_QUERY * n / (us_per_launch * 1e-6) / 1e9,
+                         # the other half of BASELINE.json's metric ("... and 1080p frame ms"), configs[2], same peak
+                         "frame_ms": frame["frame_ms"], "frame_ms_min": frame["ms_per_launch_min"],
+                         "frame_ms_max": frame["ms_per_launch_max"], "frame_frac": frame["frac"], "frame_kernel": frame["kernel"],
+                         "frame_workload": frame["workload"],
+                         "sustained": sustained},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(q_host.numel()),
                     "d2h_bytes_per_step": int(out_host.numel() * 4), "steps": k_e2e,
                     "how": f"{n_chunks} chunks per step: pinned H2D, nbsdf_eval and D2H on three streams chained by events"},
             "gpu_launches": int(launches),
             "clocks": clocks,
-            "frame": frame,
             "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": min(cores, oracle.max_threads()), "kind": "oracle", "value_1_thread": cpu_rate_1t,
                              "sample": f"all {n_cpu} queries of configs[1], {cpu_passes} passes, fp64, OpenMP over queries, {cpu_dt:.1f} s"},
         }
         line.update(extras)
+        line["frame"] = frame                                   # last on the line: a truncated tail still ends with it
     w["close"]()
     dist.finalize()
     if line is not None:

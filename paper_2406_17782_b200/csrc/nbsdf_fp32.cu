@@ -1,7 +1,11 @@
 // nbsdf_fp32.cu -- fp32 CUDA-core variant of the fused decoder (NBSDF_PREC_FP32): plain FMA, no TF32, no tensor
 // cores.  A CTA owns a tile of 256 (H = 32) or 128 (H >= 64) queries; activations live in shared memory as
-// [k][query] rows and every layer is a register-tiled product (4 x 8 outputs per thread at H = 64) with warp-uniform
-// weight loads from L1.  Accumulation runs over k in index order, like the oracle's definition, in fp32.
+// [k][query] rows and every layer is a register-tiled product (4 x 8 outputs per thread at H = 64).  For H <= 64 the
+// layer's transposed weights + bias sit in a shared-memory buffer (<= 16.6 KB) that is refilled layer by layer: the next
+// layer's chunk is fetched into registers BEFORE the current layer's FMAs and stored after them, so the inner loop is
+// LDS.128 + FMA only (round 2 read the weights with warp-uniform LDG from L1 and stalled on them: long-scoreboard 55 %
+// of samples).  H = 128 keeps the L1 path (its 196 KB of activations leave no room).  Accumulation runs over k in index
+// order, like the oracle's definition, in fp32.
 // Decoder data flow: PAPER.md:164 (sec. 4.2 "Decoder"); per-frame recipe: PAPER.md:196.
 #include "nbsdf_common.cuh"
 
@@ -63,7 +67,7 @@ constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 
 // out[n][q] = act(b[n] + sum_k Wt[k][n] in[k][q]) for n in [0, 8 TN), q in [0, 32 TQ); in/out: [.][32 TQ] floats
-template <int TQ, int TN, bool kRelu>
+template <int TQ, int TN, bool kRelu, bool kSmemW>
 __device__ __forceinline__ void dense_layer(const float* __restrict__ Wt, const float* __restrict__ b, int K,
                                             const float* in, float* out)
 {
@@ -73,7 +77,7 @@ __device__ __forceinline__ void dense_layer(const float* __restrict__ Wt, const 
     float acc[TN][TQ];
 #pragma unroll
     for (int j = 0; j < TN; ++j) {
-        const float bj = __ldg(b + n0 + j);
+        const float bj = kSmemW ? b[n0 + j] : __ldg(b + n0 + j);
 #pragma unroll
         for (int i = 0; i < TQ; ++i) acc[j][i] = bj;
     }
@@ -87,7 +91,8 @@ __device__ __forceinline__ void dense_layer(const float* __restrict__ Wt, const 
         }
 #pragma unroll
         for (int j = 0; j < TN; j += 4) {
-            const float4 v = __ldg(reinterpret_cast<const float4*>(Wt + (size_t)k * N + n0 + j));
+            const float4* wp = reinterpret_cast<const float4*>(Wt + (size_t)k * N + n0 + j);
+            const float4 v = kSmemW ? *wp : __ldg(wp);
             w[j] = v.x; w[j + 1] = v.y; w[j + 2] = v.z; w[j + 3] = v.w;
         }
 #pragma unroll
@@ -105,34 +110,93 @@ __device__ __forceinline__ void dense_layer(const float* __restrict__ Wt, const 
         }
 }
 
-// MLP-A: x = [z, u', v', lf] in bufA -> feat in bufB rows [0, F)
-template <int TQ, int TN>
-__device__ __forceinline__ void mlp_a(const NetParams& net, const Fp32Layout& lay, float* bufA, float* bufB)
+// Per-layer weight staging (kStage): chunk l = blob[w_off[l], w_off[l+1]) = transposed weights followed by the bias, a
+// multiple of 4 floats.  fetch(l) starts the global loads of chunk l into PF float4 registers per thread; commit() stores
+// them into the shared buffer (the caller has synchronised: nobody still reads the previous chunk) -- the loads'
+// latency passes under the FMAs of the layer in between.  Without kStage both are no-ops and W()/B() point into the blob.
+template <bool kStage, int PF>
+struct WStage {
+    float* wbuf;
+    const float* blob;
+    Fp32Layout lay;
+    float4 pre[PF];
+    int cur;                                              // layer whose chunk is (being put) in wbuf
+    static constexpr bool kStaged = kStage;
+
+    __device__ __forceinline__ uint32_t chunk_end(int l) const { return l == 5 ? lay.total : lay.w_off[l + 1]; }
+    __device__ __forceinline__ void fetch(int l)
+    {
+        if constexpr (kStage) {
+            const float4* src = reinterpret_cast<const float4*>(blob + lay.w_off[l]);
+            const int n4 = (int)((chunk_end(l) - lay.w_off[l]) >> 2);
+#pragma unroll
+            for (int j = 0; j < PF; ++j) {
+                const int i = threadIdx.x + j * kThreads;
+                if (i < n4) pre[j] = __ldg(src + i);
+            }
+            cur = l;
+        }
+    }
+    __device__ __forceinline__ void commit()
+    {
+        if constexpr (kStage) {
+            const int n4 = (int)((chunk_end(cur) - lay.w_off[cur]) >> 2);
+#pragma unroll
+            for (int j = 0; j < PF; ++j) {
+                const int i = threadIdx.x + j * kThreads;
+                if (i < n4) reinterpret_cast<float4*>(wbuf)[i] = pre[j];
+            }
+        }
+    }
+    __device__ __forceinline__ const float* W(int l) const { return kStage ? wbuf : blob + lay.w_off[l]; }
+    __device__ __forceinline__ const float* B(int l) const { return kStage ? wbuf + (lay.b_off[l] - lay.w_off[l]) : blob + lay.b_off[l]; }
+    // after a layer: everyone has finished reading wbuf -> store the prefetched chunk -> visible to everyone
+    __device__ __forceinline__ void turn()
+    {
+        __syncthreads();
+        if constexpr (kStage) {
+            commit();
+            __syncthreads();
+        }
+    }
+};
+
+// MLP-A: x = [z, u', v', lf] in bufA -> feat in bufB rows [0, F).  On entry wbuf holds chunk 0; on exit chunk 3.
+template <int TQ, int TN, class WS>
+__device__ __forceinline__ void mlp_a(const NetParams& net, WS& ws, float* bufA, float* bufB)
 {
-    const float* w = net.w32;
-    dense_layer<TQ, TN, true>(w + lay.w_off[0], w + lay.b_off[0], net.L + 3, bufA, bufB);
-    __syncthreads();
-    dense_layer<TQ, TN, true>(w + lay.w_off[1], w + lay.b_off[1], net.H, bufB, bufA);
-    __syncthreads();
-    dense_layer<TQ, kFeat / kWarps, false>(w + lay.w_off[2], w + lay.b_off[2], net.H, bufA, bufB);
-    __syncthreads();
+    constexpr bool S = WS::kStaged;
+    ws.fetch(1);
+    dense_layer<TQ, TN, true, S>(ws.W(0), ws.B(0), net.L + 3, bufA, bufB);
+    ws.turn();
+    ws.fetch(2);
+    dense_layer<TQ, TN, true, S>(ws.W(1), ws.B(1), net.H, bufB, bufA);
+    ws.turn();
+    ws.fetch(3);
+    dense_layer<TQ, kFeat / kWarps, false, S>(ws.W(2), ws.B(2), net.H, bufA, bufB);
+    ws.turn();
 }
 
-// MLP-B: y = [feat, wi, wo] in bufB rows [0, F+6) -> rgb of query q (threads q < 32 TQ); bufB is preserved
-template <int TQ, int TN>
-__device__ __forceinline__ void mlp_b(const NetParams& net, const Fp32Layout& lay, float* bufA, float* bufB, float* bufC,
-                                      float rgb[3])
+// MLP-B: y = [feat, wi, wo] in bufB rows [0, F+6) -> rgb of query q (threads q < 32 TQ); bufB is preserved.
+// On entry wbuf holds chunk 3; `again`: another MLP-B follows (next light), so chunk 3 is put back at the end -- the
+// caller's __syncthreads() before that next MLP-B makes it visible.
+template <int TQ, int TN, class WS>
+__device__ __forceinline__ void mlp_b(const NetParams& net, WS& ws, float* bufA, float* bufB, float* bufC, float rgb[3], bool again)
 {
     constexpr int Q = 32 * TQ;
+    constexpr bool S = WS::kStaged;
     const float* w = net.w32;
-    dense_layer<TQ, TN, true>(w + lay.w_off[3], w + lay.b_off[3], kFeat + 6, bufB, bufA);
+    ws.fetch(4);
+    dense_layer<TQ, TN, true, S>(ws.W(3), ws.B(3), kFeat + 6, bufB, bufA);
+    ws.turn();
+    if (again) ws.fetch(3);
+    dense_layer<TQ, TN, true, S>(ws.W(4), ws.B(4), net.H, bufA, bufC);
     __syncthreads();
-    dense_layer<TQ, TN, true>(w + lay.w_off[4], w + lay.b_off[4], net.H, bufA, bufC);
-    __syncthreads();
+    if (again) ws.commit();
     const int qi = threadIdx.x;
     if (qi < Q) {
-        const float* W6 = w + lay.w_off[5];
-        const float* b6 = w + lay.b_off[5];
+        const float* W6 = w + ws.lay.w_off[5];
+        const float* b6 = w + ws.lay.b_off[5];
         float o0 = 0.0f, o1 = 0.0f, o2 = 0.0f;
         for (int k = 0; k < net.H; ++k) {
             const float a = bufC[k * Q + qi];
@@ -155,6 +219,20 @@ __host__ __device__ __forceinline__ int kmax_of(int L, int H)
     return k;
 }
 
+// largest chunk (weights + bias, floats) of layers 0..4: what the staging buffer must hold
+__host__ __device__ inline uint32_t fp32_chunk_max(const Fp32Layout& lay)
+{
+    uint32_t m = 0;
+    for (int l = 0; l < 5; ++l) m = lay.w_off[l + 1] - lay.w_off[l] > m ? lay.w_off[l + 1] - lay.w_off[l] : m;
+    return m;
+}
+
+template <int TQ, int TN>
+struct Fp32Cfg {
+    static constexpr bool kStage = TN <= 8;                       // H <= 64
+    static constexpr int kPF = TN == 8 ? 5 : 2;                   // float4 per thread of the largest chunk: H=64: 1040/256, H=32: 312/256
+};
+
 template <int TQ, int TN>
 __global__ void __launch_bounds__(kThreads) eval_fp32_kernel(NetParams net, const nbsdf_query* __restrict__ q,
                                                              const float* __restrict__ frames, int64_t n,
@@ -168,6 +246,11 @@ __global__ void __launch_bounds__(kThreads) eval_fp32_kernel(NetParams net, cons
     float* bufB = bufA + kmax * Q;
     float* bufC = bufB + kmax * Q;
     const Fp32Layout lay = fp32_layout(net.L, net.H);
+    WStage<Fp32Cfg<TQ, TN>::kStage, Fp32Cfg<TQ, TN>::kPF> ws;
+    ws.wbuf = bufC + kmax * Q;
+    ws.blob = net.w32;
+    ws.lay = lay;
+    ws.fetch(0);                                                  // in flight under the input assembly
 
     // stages A1-A4: one query per thread (threads [0, Q)), straight into the [k][query] layout
     const int64_t i = (int64_t)blockIdx.x * Q + tid;
@@ -191,8 +274,9 @@ __global__ void __launch_bounds__(kThreads) eval_fp32_kernel(NetParams net, cons
         bufA[(net.L + 1) * Q + tid] = wrap01(rec.v);
         bufA[(net.L + 2) * Q + tid] = log_footprint<false>(rec.footprint);
     }
+    ws.commit();
     __syncthreads();
-    mlp_a<TQ, TN>(net, lay, bufA, bufB);
+    mlp_a<TQ, TN>(net, ws, bufA, bufB);
     if (mine) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -202,7 +286,7 @@ __global__ void __launch_bounds__(kThreads) eval_fp32_kernel(NetParams net, cons
     }
     __syncthreads();
     float rgb[3] = { 0.0f, 0.0f, 0.0f };
-    mlp_b<TQ, TN>(net, lay, bufA, bufB, bufC, rgb);
+    mlp_b<TQ, TN>(net, ws, bufA, bufB, bufC, rgb, false);
     if (live) {
         const bool bg = rec.material < 0;
         rgb_out[3 * i + 0] = bg ? 0.0f : rgb[0];
@@ -223,6 +307,11 @@ __global__ void __launch_bounds__(kThreads) shade_fp32_kernel(NetParams net, Fra
     float* bufB = bufA + kmax * Q;
     float* bufC = bufB + kmax * Q;
     const Fp32Layout lay = fp32_layout(net.L, net.H);
+    WStage<Fp32Cfg<TQ, TN>::kStage, Fp32Cfg<TQ, TN>::kPF> ws;
+    ws.wbuf = bufC + kmax * Q;
+    ws.blob = net.w32;
+    ws.lay = lay;
+    ws.fetch(0);
 
     const int64_t p = (int64_t)blockIdx.x * Q + tid;
     const bool mine = tid < Q, live = mine && p < fr.n_pixels;
@@ -243,8 +332,9 @@ __global__ void __launch_bounds__(kThreads) shade_fp32_kernel(NetParams net, Fra
         bufA[(net.L + 1) * Q + tid] = wrap01(tv.w);
         bufA[(net.L + 2) * Q + tid] = log_footprint<false>(pos.w);
     }
+    ws.commit();
     __syncthreads();
-    mlp_a<TQ, TN>(net, lay, bufA, bufB);      // once per pixel (the spatial feature does not depend on wi/wo)
+    mlp_a<TQ, TN>(net, ws, bufA, bufB);      // once per pixel (the spatial feature does not depend on wi/wo)
     if (mine) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) bufB[(kFeat + 3 + c) * Q + tid] = wo[c];
@@ -260,7 +350,7 @@ __global__ void __launch_bounds__(kThreads) shade_fp32_kernel(NetParams net, Fra
             for (int c = 0; c < 3; ++c) bufB[(kFeat + c) * Q + tid] = wi[c];
         }
         __syncthreads();
-        mlp_b<TQ, TN>(net, lay, bufA, bufB, bufC, rgb);
+        mlp_b<TQ, TN>(net, ws, bufA, bufB, bufC, rgb, l + 1 < lights.n);
         const float cs = fmaxf(wi[2], 0.0f);
 #pragma unroll
         for (int c = 0; c < 3; ++c) acc[c] = fmaf(rgb[c] * E[c], cs, acc[c]);
@@ -274,11 +364,15 @@ __global__ void __launch_bounds__(kThreads) shade_fp32_kernel(NetParams net, Fra
     }
 }
 
-template <int TQ>
-static size_t fp32_smem(const NetParams& net) { return (size_t)3 * kmax_of(net.L, net.H) * 32 * TQ * sizeof(float); }
+template <int TQ, int TN>
+static size_t fp32_smem(const NetParams& net)
+{
+    const size_t act = (size_t)3 * kmax_of(net.L, net.H) * 32 * TQ * sizeof(float);
+    return act + (Fp32Cfg<TQ, TN>::kStage ? fp32_chunk_max(fp32_layout(net.L, net.H)) * sizeof(float) : 0);
+}
 
-// H = 32: 8 queries x 4 outputs per thread; H = 64: 4 x 8 (128-query tiles: 96 KB, two CTAs per SM -- measured 16 % faster
-// than 8 x 8 with one CTA per SM); H = 128: 4 x 16 (a 128-query tile keeps three buffers in 196 KB)
+// H = 32: 8 queries x 4 outputs per thread; H = 64: 4 x 8 (128-query tiles: 96 KB + 16.3 KB of staged weights, two CTAs
+// per SM still fit: 2 x (112.3 + 1) KB <= 228 KB -- two CTAs measured 16 % faster than 8 x 8 with one CTA per SM); H = 128: 4 x 16 (a 128-query tile keeps three buffers in 196 KB)
 #define NBSDF_FP32_DISPATCH(CALL)                                  \
     switch (net.H) {                                               \
     case 32: { constexpr int TQ = 8, TN = 4; CALL; } break;        \
@@ -299,7 +393,7 @@ cudaError_t init_fp32()
 cudaError_t launch_eval_fp32(const NetParams& net, const nbsdf_query* q, const float* frames, int64_t n, float* rgb,
                              cudaStream_t s)
 {
-    NBSDF_FP32_DISPATCH((eval_fp32_kernel<TQ, TN><<<(unsigned)((n + 32 * TQ - 1) / (32 * TQ)), kThreads, fp32_smem<TQ>(net), s>>>(
+    NBSDF_FP32_DISPATCH((eval_fp32_kernel<TQ, TN><<<(unsigned)((n + 32 * TQ - 1) / (32 * TQ)), kThreads, fp32_smem<TQ, TN>(net), s>>>(
         net, q, frames, n, rgb)))
     return cudaGetLastError();
 }
@@ -308,7 +402,7 @@ cudaError_t launch_shade_fp32(const NetParams& net, const FrameParams& fr, const
                               cudaStream_t s)
 {
     NBSDF_FP32_DISPATCH((shade_fp32_kernel<TQ, TN><<<(unsigned)((fr.n_pixels + 32 * TQ - 1) / (32 * TQ)), kThreads,
-                                                   fp32_smem<TQ>(net), s>>>(net, fr, lights, out)))
+                                                   fp32_smem<TQ, TN>(net), s>>>(net, fr, lights, out)))
     return cudaGetLastError();
 }
 

@@ -373,10 +373,13 @@ static size_t fp32_smem(const NetParams& net)
 
 // H = 32: 8 queries x 4 outputs per thread; H = 64: 4 x 8 (128-query tiles: 96 KB + 16.3 KB of staged weights, two CTAs
 // per SM still fit: 2 x (112.3 + 1) KB <= 228 KB -- two CTAs measured 16 % faster than 8 x 8 with one CTA per SM); H = 128: 4 x 16 (a 128-query tile keeps three buffers in 196 KB)
+#ifndef NBSDF_FP32_TQ64
+#define NBSDF_FP32_TQ64 4
+#endif
 #define NBSDF_FP32_DISPATCH(CALL)                                  \
     switch (net.H) {                                               \
     case 32: { constexpr int TQ = 8, TN = 4; CALL; } break;        \
-    case 64: { constexpr int TQ = 4, TN = 8; CALL; } break; \
+    case 64: { constexpr int TQ = NBSDF_FP32_TQ64, TN = 8; CALL; } break; \
     case 128: { constexpr int TQ = 4, TN = 16; CALL; } break;      \
     default: return cudaErrorInvalidValue;                         \
     }
@@ -384,9 +387,9 @@ static size_t fp32_smem(const NetParams& net)
 cudaError_t init_fp32()
 {
     cudaError_t e = cudaSuccess;
-    auto set = [&](const void* k) { if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); };
-    set((const void*)eval_fp32_kernel<8, 4>); set((const void*)eval_fp32_kernel<4, 8>); set((const void*)eval_fp32_kernel<4, 16>);
-    set((const void*)shade_fp32_kernel<8, 4>); set((const void*)shade_fp32_kernel<4, 8>); set((const void*)shade_fp32_kernel<4, 16>);
+    auto set = [&](const void* k) { if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); };
+    set((const void*)eval_fp32_kernel<8, 4>); set((const void*)eval_fp32_kernel<NBSDF_FP32_TQ64, 8>); set((const void*)eval_fp32_kernel<4, 16>);
+    set((const void*)shade_fp32_kernel<8, 4>); set((const void*)shade_fp32_kernel<NBSDF_FP32_TQ64, 8>); set((const void*)shade_fp32_kernel<4, 16>);
     return e;
 }
 
